@@ -1,0 +1,175 @@
+/*
+ * microlens.h -- C ABI of the B200-native direct inverse ray-shooting library.
+ *
+ * What it computes (citations: /root/reference/PAPER.md line, section/equation):
+ *   A regular grid of light rays covering an image-plane "shooting rectangle" is
+ *   propagated backwards through a lens plane of N* unit-mass point lenses plus a
+ *   smooth convergence sigma_c and an external shear gamma (eq.4):
+ *
+ *       y1 = (1 - gamma - sigma_c) x1 - sum_i (x1 - xi1)/|x - xi|^2
+ *       y2 = (1 + gamma - sigma_c) x2 - sum_i (x2 - xi2)/|x - xi|^2
+ *
+ *   and each ray is counted into the source-plane pixel it reaches; the map of
+ *   counts N_ij gives the magnification mu_ij = N_ij / N_rays (eq.3).
+ *   This is the "GPU-D" direct code of PAPER.md:119-138 (section 2.3), redesigned: rays are
+ *   generated in-kernel from their grid index, deflected by an all-pairs FP32 sum
+ *   over shared-memory lens tiles, and binned by warp-aggregated atomics in the
+ *   same kernel.  Lengths are in Einstein radii of one lens; masses are 1
+ *   (PAPER.md:165).
+ *
+ * Conventions
+ *   - Every function returns an int: ML_OK (0) or a negative ML_ERR_* code.  The
+ *     library never throws, aborts or prints.  ml_strerror() names a code.
+ *   - "host" / "device" below says where a pointer must live.  The caller owns
+ *     every buffer it passes; the library copies what it needs before returning.
+ *   - A context is not thread-safe; separate contexts are independent.
+ *   - There is no CPU fallback: without a CUDA device ml_create fails with
+ *     ML_ERR_CUDA.
+ *
+ * Geometry derived by ml_create (all fp64; DESIGN.md "Readings" R1-R8):
+ *   kappa_star = stellar_fraction*sigma, kappa_c = sigma - kappa_star
+ *   pixel = L/n_pix;  ray spacing delta = pixel/sqrt(n_rays)
+ *   a1 = 1.2 (L/2)/|1-sigma-gamma|, a2 = 1.2 (L/2)/|1-sigma+gamma|      (eq.11)
+ *   n1 = ceil(2 a1/delta - 1e-9), n2 likewise; ray (i,j), 0<=i<n1, 0<=j<n2, sits at
+ *   x = ((i-(n1-1)/2) delta, (j-(n2-1)/2) delta)
+ *   R* = 1.3 sqrt(a1^2+a2^2);  N*_expected = floor(kappa_star R*^2 + 0.5) (eq.5)
+ *   pixel (i',j') of y: i' = floor((y1+L/2)/pixel), j' = floor((y2+L/2)/pixel);
+ *   counted iff 0 <= i',j' < n_pix.  Map layout: map[j'*n_pix + i'] (uint32).
+ */
+#ifndef MICROLENS_H
+#define MICROLENS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ml_ctx ml_ctx; /* opaque */
+
+enum {
+    ML_OK = 0,
+    ML_ERR_INVALID_ARG = -1, /* bad argument (see each call)                        */
+    ML_ERR_CUDA = -2,        /* a CUDA runtime call failed / no device              */
+    ML_ERR_OOM = -3,         /* host or device allocation failed                    */
+    ML_ERR_STATE = -4        /* call sequence error (e.g. shoot before set_lenses)  */
+};
+
+/* Arithmetic of the deflection sum (eq.8 leaves the summation order open;
+ * DESIGN.md "Summation order and precision" fixes it for each mode). */
+enum {
+    ML_PREC_FP32_TILED = 0,       /* default: tile-local FP32 terms, FP32 partial sums over K
+                                     lenses flushed into fp64 accumulators, fp64 epilogue    */
+    ML_PREC_FP32_COMPENSATED = 1, /* as above, Newton-refined reciprocal and a flush every
+                                     8 lenses                                                */
+    ML_PREC_FP64 = 2              /* everything in fp64 (true division)                      */
+};
+
+typedef struct {
+    double kappa_star, kappa_c;      /* sigma_*, sigma_c                                    */
+    double a1, a2;                   /* half-sides of the shooting rectangle (R_E)          */
+    double ray_spacing;              /* delta                                               */
+    double r_star;                   /* lens-disk radius R*                                 */
+    double pixel_side;               /* L / n_pix                                           */
+    double mu_theory;                /* 1/((1-sigma)^2-gamma^2), signed (eq.12) */
+    int64_t n1, n2;                  /* rays along axis 1 / axis 2                          */
+    int64_t n_star_expected;         /* N* of eq.5 for the disk above                       */
+    int64_t n_lenses;                /* lenses currently set (-1 before ml_set_lenses)      */
+    int32_t n_pix;                   /* pixels per side                                     */
+    int32_t tile_w, tile_h;          /* ray tile of one CTA in the current precision mode   */
+    int32_t precision;               /* ML_PREC_*                                           */
+    int32_t device;                  /* CUDA device ordinal                                 */
+    int32_t sm_count;                /* multiProcessorCount of that device                  */
+    int32_t sm_clock_khz;            /* cudaDevAttrClockRate (max SM clock)                 */
+} ml_info;
+
+typedef struct {
+    uint64_t rays_shot;    /* rays processed by the last shoot (sum over accumulated regions) */
+    uint64_t rays_in_map;  /* rays counted into the map                                       */
+    uint64_t rays_dropped; /* rays whose y was not finite (ray on a lens): not binned         */
+    uint64_t interactions; /* rays_shot * n_lenses (eq.6 without N_FLOP)       */
+    uint64_t kernel_launches; /* launches of the shoot kernel since the map was last zeroed   */
+    double kernel_ms;      /* device time of those launches, CUDA events on the ctx stream    */
+    double total_ms;       /* host wall time of the last ml_shoot / ml_shoot_region call      */
+} ml_stats;
+
+/* Create a context for one map.  Arguments are the paper's statement of the problem
+ * (PAPER.md:152-158, :25): total convergence sigma, stellar fraction sigma_* / sigma
+ * (= 1 - s of PAPER.md:158), shear gamma, pixels per side n_pix, mean rays per pixel
+ * n_rays, source-plane side L (Einstein radii); `device` is the CUDA ordinal.
+ * Allocates the n_pix^2 uint32 device map.  *out is owned by the library until
+ * ml_destroy.  ML_ERR_INVALID_ARG if out is NULL, any value is not finite, sigma < 0,
+ * stellar_fraction outside [0,1], n_pix <= 0 or > 32768, n_rays <= 0, L <= 0,
+ * |1-sigma-gamma| or |1-sigma+gamma| < 1e-6 (critical line: unbounded rectangle,
+ * PAPER.md:285) or n1*n2 >= 2^62. */
+int ml_create(double sigma, double stellar_fraction, double gamma, int32_t n_pix,
+              double n_rays, double L, int32_t device, ml_ctx **out);
+
+/* Frees everything.  NULL is a no-op. */
+void ml_destroy(ml_ctx *ctx);
+
+/* Derived geometry and device facts (host struct filled). */
+int ml_get_info(const ml_ctx *ctx, ml_info *out);
+
+/* Lens positions (PAPER.md:130 step 1, :138): xy = n interleaved (x, y) HOST fp64
+ * pairs in Einstein radii, unit masses.  Copied to the device; the caller keeps xy.
+ * n >= 0 and need not equal n_star_expected (n = 0: no stars).  A non-finite
+ * coordinate gives ML_ERR_INVALID_ARG and leaves the previous lenses in place. */
+int ml_set_lenses(ml_ctx *ctx, const double *xy, int64_t n);
+
+/* Select ML_PREC_*; ML_ERR_INVALID_ARG for any other value. */
+int ml_set_precision(ml_ctx *ctx, int mode);
+
+/* Zero the map and the statistics, shoot the whole n1 x n2 grid (PAPER.md:128-136 steps
+ * 2-7 as one fused kernel per <= 2^31-1 tiles), synchronise.  ML_ERR_STATE before
+ * ml_set_lenses. */
+int ml_shoot(ml_ctx *ctx);
+
+/* Same for the ray-index rectangle [i0,i1) x [j0,j1) only.  accumulate = 0 zeroes the
+ * map and statistics first; != 0 adds to them.  Tiles are aligned to the global
+ * grid, so a ray's arithmetic does not depend on the region it is shot in: any
+ * partition of the grid into regions gives bit-identical counts to ml_shoot.
+ * ML_ERR_INVALID_ARG unless 0 <= i0 <= i1 <= n1 and 0 <= j0 <= j1 <= n2. */
+int ml_shoot_region(ml_ctx *ctx, int64_t i0, int64_t i1, int64_t j0, int64_t j1, int accumulate);
+
+/* Copy the n_pix^2 counts to a HOST buffer of out_len >= n_pix^2 elements
+ * (else ML_ERR_INVALID_ARG).  out[j'*n_pix + i'], i' <-> y1 (fast), j' <-> y2. */
+int ml_get_map(const ml_ctx *ctx, uint32_t *out, size_t out_len);
+
+/* Borrowed DEVICE pointer to the map (valid until ml_destroy / ml_use_device_map). */
+int ml_get_map_device(const ml_ctx *ctx, void **dptr);
+
+/* Use caller-owned DEVICE memory (>= n_pix^2 uint32, e.g. a torch tensor) as the map
+ * from now on; NULL returns to the library's own buffer.  The caller keeps ownership. */
+int ml_use_device_map(ml_ctx *ctx, void *dptr);
+
+/* Launch on this CUDA stream (a cudaStream_t as void*, e.g. torch's current stream;
+ * NULL = the legacy default stream) instead of the context's own. */
+int ml_attach_stream(ml_ctx *ctx, void *cuda_stream);
+
+/* Counters and timings of the last shoot. */
+int ml_get_stats(const ml_ctx *ctx, ml_stats *out);
+
+/* Source-plane position (y1, y2) of EVERY ray of [i0,i1) x [j0,j1), computed by the
+ * shoot kernel itself (same tile membership, summation order and epilogue; the
+ * capture instantiation stores y instead of binning).  y_out = HOST buffer of
+ * 2*(i1-i0)*(j1-j0) doubles, y_out[2*((j-j0)*(i1-i0) + (i-i0)) + {0,1}]; a dropped
+ * ray gives NaN.  Does not touch the map.  ML_ERR_INVALID_ARG for a bad region,
+ * ML_ERR_OOM if (i1-i0)*(j1-j0) > 2^28 rays. */
+int ml_capture_region(ml_ctx *ctx, int64_t i0, int64_t i1, int64_t j0, int64_t j1, double *y_out);
+
+/* Same for n listed rays (HOST int64 arrays ray_i, ray_j): y_out[2k], y_out[2k+1].
+ * Cost: one whole tile per distinct tile touched. */
+int ml_probe(ml_ctx *ctx, int64_t n, const int64_t *ray_i, const int64_t *ray_j, double *y_out);
+
+/* Static description of a return code. */
+const char *ml_strerror(int code);
+
+/* Library version string, e.g. "microlens-b200 0.1 (sm_100a)". */
+const char *ml_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MICROLENS_H */

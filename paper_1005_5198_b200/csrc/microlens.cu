@@ -1,0 +1,500 @@
+// microlens.cu -- host side of the C ABI declared in include/microlens.h.
+//
+// Holds the problem geometry (PAPER.md:56-60 eq.5, :275-285 eq.11, :287-292 eq.12 with the
+// concrete rules of BASELINE.json:configs[0]; readings R1-R8), the device
+// buffers and the launch logic.  All arithmetic on rays happens in shoot_kernel.cuh.
+// There is no CPU path: every entry point that computes needs a CUDA device.
+#include "../../include/microlens.h"
+#include "shoot_kernel.cuh"
+
+#include <algorithm>
+#include <chrono>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace mlb200;
+
+struct ml_ctx {
+    // problem statement
+    double sigma, stellar_fraction, gamma, n_rays, L;
+    int32_t n_pix;
+    // derived
+    double kappa_star, kappa_c, pixel, delta, a1, a2, r_star, mu_th;
+    int64_t n1, n2, n_star_expected;
+    // device state
+    int device;
+    int sm_count, sm_clock_khz;
+    cudaStream_t own_stream, stream;
+    cudaEvent_t ev0, ev1;
+    unsigned int *map_own, *map;
+    double2 *lens;
+    int64_t n_lenses; // -1: never set
+    unsigned long long *counters; // device [3]
+    int precision;
+    ml_stats stats;
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev;
+    bool ok;
+    explicit DeviceGuard(int dev) : prev(0), ok(false)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) return;
+        ok = (prev == dev) || (cudaSetDevice(dev) == cudaSuccess);
+    }
+    ~DeviceGuard()
+    {
+        if (ok) cudaSetDevice(prev);
+    }
+};
+
+// Tile shape and kernel instantiations per precision mode.
+struct Mode {
+    int tw, th;
+};
+constexpr int RXF = 4, RYF = 4, KFF = 64;  // FP32_TILED
+constexpr int KFC = 8;                     // FP32_COMPENSATED
+constexpr int RXD = 2, RYD = 2, KFD = 64;  // FP64
+
+Mode mode_of(int precision)
+{
+    if (precision == ML_PREC_FP64) return {32 * RXD, kWarps * RYD};
+    return {32 * RXF, kWarps * RYF};
+}
+
+template <bool CAPTURE> cudaError_t launch(int precision, long long n_tiles, const ShootParams &p, cudaStream_t s)
+{
+    if (n_tiles <= 0) return cudaSuccess;
+    const unsigned int g = (unsigned int)n_tiles;
+    switch (precision) {
+    case ML_PREC_FP64:
+        shoot_kernel<double, RXD, RYD, KFD, false, CAPTURE><<<g, kThreads, 0, s>>>(p);
+        break;
+    case ML_PREC_FP32_COMPENSATED:
+        shoot_kernel<float, RXF, RYF, KFC, true, CAPTURE><<<g, kThreads, 0, s>>>(p);
+        break;
+    default:
+        shoot_kernel<float, RXF, RYF, KFF, false, CAPTURE><<<g, kThreads, 0, s>>>(p);
+        break;
+    }
+    return cudaGetLastError();
+}
+
+ShootParams base_params(const ml_ctx *c)
+{
+    ShootParams p;
+    std::memset(&p, 0, sizeof(p));
+    p.lens = c->lens;
+    p.n_lens = (int)c->n_lenses;
+    p.n_pix = c->n_pix;
+    p.delta = c->delta;
+    p.half1 = (double)(c->n1 - 1) / 2.0;
+    p.half2 = (double)(c->n2 - 1) / 2.0;
+    p.c1 = 1.0 - c->gamma - c->kappa_c;
+    p.c2 = 1.0 + c->gamma - c->kappa_c;
+    p.halfL = c->L / 2.0;
+    p.inv_pixel = (double)c->n_pix / c->L;
+    p.map = c->map;
+    p.counters = c->counters;
+    return p;
+}
+
+constexpr long long kMaxTilesPerLaunch = 0x7fffffffLL;
+
+int shoot_region_impl(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1, int accumulate)
+{
+    if (!c) return ML_ERR_INVALID_ARG;
+    if (c->n_lenses < 0) return ML_ERR_STATE;
+    if (i0 < 0 || j0 < 0 || i1 > c->n1 || j1 > c->n2 || i0 > i1 || j0 > j1) return ML_ERR_INVALID_ARG;
+    DeviceGuard g(c->device);
+    if (!g.ok) return ML_ERR_CUDA;
+    const auto t0 = std::chrono::steady_clock::now();
+    if (!accumulate) {
+        if (cudaMemsetAsync(c->map, 0, (size_t)c->n_pix * c->n_pix * sizeof(unsigned int), c->stream) != cudaSuccess ||
+            cudaMemsetAsync(c->counters, 0, 3 * sizeof(unsigned long long), c->stream) != cudaSuccess)
+            return ML_ERR_CUDA;
+        std::memset(&c->stats, 0, sizeof(c->stats));
+    }
+    float ms = 0.f;
+    uint64_t launches = 0;
+    if (i1 > i0 && j1 > j0) {
+        const Mode m = mode_of(c->precision);
+        ShootParams p = base_params(c);
+        p.i0 = i0; p.i1 = i1; p.j0 = j0; p.j1 = j1;
+        p.tile_i0 = i0 / m.tw;
+        p.tile_j0 = j0 / m.th;
+        p.tiles_x = (i1 - 1) / m.tw - p.tile_i0 + 1;
+        const long long tiles_y = (j1 - 1) / m.th - p.tile_j0 + 1;
+        const long long n_tiles = p.tiles_x * tiles_y;
+        if (cudaEventRecord(c->ev0, c->stream) != cudaSuccess) return ML_ERR_CUDA;
+        for (long long base = 0; base < n_tiles; base += kMaxTilesPerLaunch) {
+            p.tile_base = base;
+            if (launch<false>(c->precision, std::min(kMaxTilesPerLaunch, n_tiles - base), p, c->stream) != cudaSuccess)
+                return ML_ERR_CUDA;
+            ++launches;
+        }
+        if (cudaEventRecord(c->ev1, c->stream) != cudaSuccess) return ML_ERR_CUDA;
+    }
+    unsigned long long h[3];
+    if (cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess)
+        return ML_ERR_CUDA;
+    if (launches && cudaEventElapsedTime(&ms, c->ev0, c->ev1) != cudaSuccess) return ML_ERR_CUDA;
+    c->stats.rays_shot = h[0];
+    c->stats.rays_in_map = h[1];
+    c->stats.rays_dropped = h[2];
+    c->stats.interactions = h[0] * (uint64_t)c->n_lenses;
+    c->stats.kernel_launches += launches;
+    c->stats.kernel_ms += ms;
+    c->stats.total_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
+    return ML_OK;
+}
+
+// Run the capture instantiation on an explicit list of global tiles and hand every
+// batch of results to `sink(first_tile_in_list, n_tiles_in_batch, host_buffer)`.
+template <typename Sink>
+int capture_tiles(ml_ctx *c, const std::vector<long long> &tiles /* pairs */, Sink sink)
+{
+    const Mode m = mode_of(c->precision);
+    const size_t per_tile = (size_t)m.tw * m.th;
+    const long long n_tiles = (long long)(tiles.size() / 2);
+    if (n_tiles == 0) return ML_OK;
+    const long long batch = std::max<long long>(1, std::min<long long>(n_tiles, (256ll << 20) / (long long)(per_tile * sizeof(double2))));
+    long long *d_list = nullptr;
+    double2 *d_buf = nullptr;
+    std::vector<double2> h_buf;
+    try {
+        h_buf.resize((size_t)batch * per_tile);
+    } catch (const std::bad_alloc &) {
+        return ML_ERR_OOM;
+    }
+    int rc = ML_OK;
+    if (cudaMalloc(&d_list, tiles.size() * sizeof(long long)) != cudaSuccess ||
+        cudaMalloc(&d_buf, (size_t)batch * per_tile * sizeof(double2)) != cudaSuccess) {
+        cudaGetLastError();
+        rc = ML_ERR_OOM;
+    }
+    if (rc == ML_OK && cudaMemcpyAsync(d_list, tiles.data(), tiles.size() * sizeof(long long), cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+        rc = ML_ERR_CUDA;
+    for (long long first = 0; rc == ML_OK && first < n_tiles; first += batch) {
+        const long long nb = std::min(batch, n_tiles - first);
+        ShootParams p = base_params(c);
+        p.capture = d_buf;
+        p.tile_list = d_list + 2 * first;
+        p.tile_base = 0;
+        if (launch<true>(c->precision, nb, p, c->stream) != cudaSuccess ||
+            cudaMemcpyAsync(h_buf.data(), d_buf, (size_t)nb * per_tile * sizeof(double2), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+            cudaStreamSynchronize(c->stream) != cudaSuccess) {
+            rc = ML_ERR_CUDA;
+            break;
+        }
+        sink(first, nb, h_buf.data());
+    }
+    cudaFree(d_list);
+    cudaFree(d_buf);
+    return rc;
+}
+
+} // namespace
+
+extern "C" {
+
+int ml_create(double sigma, double stellar_fraction, double gamma, int32_t n_pix, double n_rays, double L,
+              int32_t device, ml_ctx **out)
+{
+    if (!out) return ML_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!std::isfinite(sigma) || !std::isfinite(stellar_fraction) || !std::isfinite(gamma) || !std::isfinite(n_rays) ||
+        !std::isfinite(L))
+        return ML_ERR_INVALID_ARG;
+    if (sigma < 0.0 || stellar_fraction < 0.0 || stellar_fraction > 1.0 || n_pix <= 0 || n_pix > 32768 ||
+        n_rays <= 0.0 || L <= 0.0)
+        return ML_ERR_INVALID_ARG;
+    const double minus = 1.0 - sigma - gamma, plus = 1.0 - sigma + gamma;
+    if (std::fabs(minus) < 1e-6 || std::fabs(plus) < 1e-6) return ML_ERR_INVALID_ARG;
+
+    ml_ctx *c = new (std::nothrow) ml_ctx;
+    if (!c) return ML_ERR_OOM;
+    std::memset(c, 0, sizeof(*c));
+    c->sigma = sigma; c->stellar_fraction = stellar_fraction; c->gamma = gamma;
+    c->n_rays = n_rays; c->L = L; c->n_pix = n_pix;
+    c->kappa_star = stellar_fraction * sigma;
+    c->kappa_c = sigma - c->kappa_star;
+    c->pixel = L / (double)n_pix;
+    c->delta = c->pixel / std::sqrt(n_rays);
+    c->a1 = 1.2 * (L / 2.0) / std::fabs(minus);
+    c->a2 = 1.2 * (L / 2.0) / std::fabs(plus);
+    const double f1 = std::ceil(2.0 * c->a1 / c->delta - 1e-9), f2 = std::ceil(2.0 * c->a2 / c->delta - 1e-9);
+    if (!(f1 >= 1.0) || !(f2 >= 1.0) || f1 * f2 >= 4.611686018427388e18 || f1 >= 9.0e15 || f2 >= 9.0e15) {
+        delete c;
+        return ML_ERR_INVALID_ARG;
+    }
+    c->n1 = (int64_t)f1;
+    c->n2 = (int64_t)f2;
+    c->r_star = 1.3 * std::sqrt(c->a1 * c->a1 + c->a2 * c->a2);
+    c->n_star_expected = (int64_t)std::floor(c->kappa_star * c->r_star * c->r_star + 0.5);
+    c->mu_th = 1.0 / ((1.0 - sigma) * (1.0 - sigma) - gamma * gamma);
+    c->n_lenses = -1;
+    c->precision = ML_PREC_FP32_TILED;
+    c->device = device;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        delete c;
+        return ML_ERR_CUDA;
+    }
+    DeviceGuard g(device);
+    int rc = g.ok ? ML_OK : ML_ERR_CUDA;
+    if (rc == ML_OK &&
+        (cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
+         cudaDeviceGetAttribute(&c->sm_clock_khz, cudaDevAttrClockRate, device) != cudaSuccess ||
+         cudaStreamCreateWithFlags(&c->own_stream, cudaStreamNonBlocking) != cudaSuccess ||
+         cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess))
+        rc = ML_ERR_CUDA;
+    if (rc == ML_OK) {
+        c->stream = c->own_stream;
+        if (cudaMalloc(&c->map_own, (size_t)n_pix * n_pix * sizeof(unsigned int)) != cudaSuccess ||
+            cudaMalloc(&c->counters, 3 * sizeof(unsigned long long)) != cudaSuccess) {
+            cudaGetLastError();
+            rc = ML_ERR_OOM;
+        }
+    }
+    if (rc == ML_OK) {
+        c->map = c->map_own;
+        if (cudaMemsetAsync(c->map, 0, (size_t)n_pix * n_pix * sizeof(unsigned int), c->stream) != cudaSuccess ||
+            cudaMemsetAsync(c->counters, 0, 3 * sizeof(unsigned long long), c->stream) != cudaSuccess ||
+            cudaStreamSynchronize(c->stream) != cudaSuccess)
+            rc = ML_ERR_CUDA;
+    }
+    if (rc != ML_OK) {
+        ml_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return ML_OK;
+}
+
+void ml_destroy(ml_ctx *c)
+{
+    if (!c) return;
+    {
+        DeviceGuard g(c->device);
+        if (g.ok) {
+            if (c->own_stream) cudaStreamSynchronize(c->own_stream);
+            if (c->map_own) cudaFree(c->map_own);
+            if (c->lens) cudaFree(c->lens);
+            if (c->counters) cudaFree(c->counters);
+            if (c->ev0) cudaEventDestroy(c->ev0);
+            if (c->ev1) cudaEventDestroy(c->ev1);
+            if (c->own_stream) cudaStreamDestroy(c->own_stream);
+        }
+    }
+    delete c;
+}
+
+int ml_get_info(const ml_ctx *c, ml_info *o)
+{
+    if (!c || !o) return ML_ERR_INVALID_ARG;
+    std::memset(o, 0, sizeof(*o));
+    o->kappa_star = c->kappa_star; o->kappa_c = c->kappa_c;
+    o->a1 = c->a1; o->a2 = c->a2;
+    o->ray_spacing = c->delta; o->r_star = c->r_star; o->pixel_side = c->pixel; o->mu_theory = c->mu_th;
+    o->n1 = c->n1; o->n2 = c->n2; o->n_star_expected = c->n_star_expected; o->n_lenses = c->n_lenses;
+    o->n_pix = c->n_pix;
+    const Mode m = mode_of(c->precision);
+    o->tile_w = m.tw; o->tile_h = m.th;
+    o->precision = c->precision; o->device = c->device;
+    o->sm_count = c->sm_count; o->sm_clock_khz = c->sm_clock_khz;
+    return ML_OK;
+}
+
+int ml_set_lenses(ml_ctx *c, const double *xy, int64_t n)
+{
+    if (!c || n < 0 || n > 0x7fffff00LL || (n > 0 && !xy)) return ML_ERR_INVALID_ARG;
+    for (int64_t k = 0; k < 2 * n; ++k)
+        if (!std::isfinite(xy[k])) return ML_ERR_INVALID_ARG;
+    DeviceGuard g(c->device);
+    if (!g.ok) return ML_ERR_CUDA;
+    double2 *d = nullptr;
+    if (cudaMalloc(&d, (size_t)std::max<int64_t>(n, 1) * sizeof(double2)) != cudaSuccess) {
+        cudaGetLastError();
+        return ML_ERR_OOM;
+    }
+    if (n > 0 && (cudaMemcpyAsync(d, xy, (size_t)n * sizeof(double2), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+                  cudaStreamSynchronize(c->stream) != cudaSuccess)) {
+        cudaFree(d);
+        return ML_ERR_CUDA;
+    }
+    if (c->lens) cudaFree(c->lens);
+    c->lens = d;
+    c->n_lenses = n;
+    return ML_OK;
+}
+
+int ml_set_precision(ml_ctx *c, int mode)
+{
+    if (!c || (mode != ML_PREC_FP32_TILED && mode != ML_PREC_FP32_COMPENSATED && mode != ML_PREC_FP64))
+        return ML_ERR_INVALID_ARG;
+    c->precision = mode;
+    return ML_OK;
+}
+
+int ml_shoot(ml_ctx *c)
+{
+    if (!c) return ML_ERR_INVALID_ARG;
+    return shoot_region_impl(c, 0, c->n1, 0, c->n2, 0);
+}
+
+int ml_shoot_region(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1, int accumulate)
+{
+    return shoot_region_impl(c, i0, i1, j0, j1, accumulate);
+}
+
+int ml_get_map(const ml_ctx *c, uint32_t *out, size_t out_len)
+{
+    if (!c || !out || out_len < (size_t)c->n_pix * c->n_pix) return ML_ERR_INVALID_ARG;
+    DeviceGuard g(c->device);
+    if (!g.ok) return ML_ERR_CUDA;
+    if (cudaMemcpyAsync(out, c->map, (size_t)c->n_pix * c->n_pix * sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+        cudaStreamSynchronize(c->stream) != cudaSuccess)
+        return ML_ERR_CUDA;
+    return ML_OK;
+}
+
+int ml_get_map_device(const ml_ctx *c, void **dptr)
+{
+    if (!c || !dptr) return ML_ERR_INVALID_ARG;
+    *dptr = c->map;
+    return ML_OK;
+}
+
+int ml_use_device_map(ml_ctx *c, void *dptr)
+{
+    if (!c) return ML_ERR_INVALID_ARG;
+    c->map = dptr ? (unsigned int *)dptr : c->map_own;
+    return ML_OK;
+}
+
+int ml_attach_stream(ml_ctx *c, void *cuda_stream)
+{
+    if (!c) return ML_ERR_INVALID_ARG;
+    c->stream = (cudaStream_t)cuda_stream;
+    return ML_OK;
+}
+
+int ml_get_stats(const ml_ctx *c, ml_stats *o)
+{
+    if (!c || !o) return ML_ERR_INVALID_ARG;
+    *o = c->stats;
+    return ML_OK;
+}
+
+int ml_capture_region(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1, double *y_out)
+{
+    if (!c) return ML_ERR_INVALID_ARG;
+    if (c->n_lenses < 0) return ML_ERR_STATE;
+    if (i0 < 0 || j0 < 0 || i1 > c->n1 || j1 > c->n2 || i0 > i1 || j0 > j1) return ML_ERR_INVALID_ARG;
+    if (i1 == i0 || j1 == j0) return ML_OK;
+    if (!y_out) return ML_ERR_INVALID_ARG;
+    if ((double)(i1 - i0) * (double)(j1 - j0) > 268435456.0) return ML_ERR_OOM;
+    DeviceGuard g(c->device);
+    if (!g.ok) return ML_ERR_CUDA;
+    const Mode m = mode_of(c->precision);
+    std::vector<long long> tiles;
+    try {
+        for (long long tj = j0 / m.th; tj <= (j1 - 1) / m.th; ++tj)
+            for (long long ti = i0 / m.tw; ti <= (i1 - 1) / m.tw; ++ti) {
+                tiles.push_back(ti);
+                tiles.push_back(tj);
+            }
+    } catch (const std::bad_alloc &) {
+        return ML_ERR_OOM;
+    }
+    const int64_t w = i1 - i0;
+    return capture_tiles(c, tiles, [&](long long first, long long nb, const double2 *buf) {
+        for (long long q = 0; q < nb; ++q) {
+            const long long ti = tiles[2 * (first + q)], tj = tiles[2 * (first + q) + 1];
+            const double2 *tb = buf + (size_t)q * m.tw * m.th;
+            for (int ly = 0; ly < m.th; ++ly) {
+                const int64_t j = tj * m.th + ly;
+                if (j < j0 || j >= j1) continue;
+                for (int lx = 0; lx < m.tw; ++lx) {
+                    const int64_t i = ti * m.tw + lx;
+                    if (i < i0 || i >= i1) continue;
+                    const double2 v = tb[(size_t)ly * m.tw + lx];
+                    double *o = y_out + 2 * ((j - j0) * w + (i - i0));
+                    o[0] = v.x;
+                    o[1] = v.y;
+                }
+            }
+        }
+    });
+}
+
+int ml_probe(ml_ctx *c, int64_t n, const int64_t *ray_i, const int64_t *ray_j, double *y_out)
+{
+    if (!c || n < 0) return ML_ERR_INVALID_ARG;
+    if (c->n_lenses < 0) return ML_ERR_STATE;
+    if (n == 0) return ML_OK;
+    if (!ray_i || !ray_j || !y_out) return ML_ERR_INVALID_ARG;
+    for (int64_t k = 0; k < n; ++k)
+        if (ray_i[k] < 0 || ray_i[k] >= c->n1 || ray_j[k] < 0 || ray_j[k] >= c->n2) return ML_ERR_INVALID_ARG;
+    DeviceGuard g(c->device);
+    if (!g.ok) return ML_ERR_CUDA;
+    const Mode m = mode_of(c->precision);
+    // rays sorted by the tile that owns them; one capture tile per distinct tile
+    std::vector<int64_t> order;
+    std::vector<long long> tiles;
+    std::vector<int64_t> first_ray_of_tile; // index into `order`
+    try {
+        order.resize((size_t)n);
+        for (int64_t k = 0; k < n; ++k) order[(size_t)k] = k;
+        auto key = [&](int64_t k) { return std::make_pair(ray_j[k] / m.th, ray_i[k] / m.tw); };
+        std::sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return key(a) < key(b); });
+        for (int64_t q = 0; q < n; ++q) {
+            const int64_t k = order[(size_t)q];
+            const long long ti = ray_i[k] / m.tw, tj = ray_j[k] / m.th;
+            if (tiles.empty() || tiles[tiles.size() - 2] != ti || tiles[tiles.size() - 1] != tj) {
+                tiles.push_back(ti);
+                tiles.push_back(tj);
+                first_ray_of_tile.push_back(q);
+            }
+        }
+        first_ray_of_tile.push_back(n);
+    } catch (const std::bad_alloc &) {
+        return ML_ERR_OOM;
+    }
+    return capture_tiles(c, tiles, [&](long long first, long long nb, const double2 *buf) {
+        for (long long q = 0; q < nb; ++q) {
+            const long long ti = tiles[2 * (first + q)], tj = tiles[2 * (first + q) + 1];
+            const double2 *tb = buf + (size_t)q * m.tw * m.th;
+            for (int64_t s = first_ray_of_tile[(size_t)(first + q)]; s < first_ray_of_tile[(size_t)(first + q) + 1]; ++s) {
+                const int64_t k = order[(size_t)s];
+                const double2 v = tb[(size_t)(ray_j[k] - tj * m.th) * m.tw + (size_t)(ray_i[k] - ti * m.tw)];
+                y_out[2 * k] = v.x;
+                y_out[2 * k + 1] = v.y;
+            }
+        }
+    });
+}
+
+const char *ml_strerror(int code)
+{
+    switch (code) {
+    case ML_OK: return "ok";
+    case ML_ERR_INVALID_ARG: return "invalid argument";
+    case ML_ERR_CUDA: return "CUDA runtime error or no CUDA device";
+    case ML_ERR_OOM: return "out of memory";
+    case ML_ERR_STATE: return "call sequence error (lenses not set)";
+    default: return "unknown error code";
+    }
+}
+
+const char *ml_version(void) { return "microlens-b200 0.1 (sm_100a)"; }
+
+} // extern "C"

@@ -1,0 +1,277 @@
+// shoot_kernel.cuh -- the fused ray-generation + deflection + binning kernel (sm_100a).
+//
+// One CTA shoots one tile of TW x TH rays of the regular image-plane grid through all
+// N* lenses (eq.4, unit masses PAPER.md:165) and bins them into the
+// source-plane count map (eq.3).  Steps a1-a6 of SURVEY.md section 8(a):
+//
+//   a1 lens staging   lens positions (fp64, L2-resident) are re-centred on the tile centre
+//                     with an fp64 subtract, rounded to the working type and staged into
+//                     shared memory in chunks of CHUNK lenses, double-buffered: global loads
+//                     for chunk n+1 are issued before the arithmetic on chunk n.
+//   a2 ray generation ray (i,j) -> x from the tile / thread index; nothing is stored.
+//   a3 deflection     each thread owns an RX x RY block of rays; per lens the RX column
+//                     differences / squares and RY row differences / squares are shared, so
+//                     one interaction is FADD (r^2) + MUFU.RCP + 2 FFMA, plus
+//                     2(RX+RY)/(RX*RY) amortised FADD/FMUL.
+//   a4 macro terms    y = (1 -/+ gamma - kappa_c) x - S in fp64.
+//   a5 binning        pixel index in fp64; per register slot the 32 lanes of a warp hold 32
+//                     rays of one row, RX apart: runs of equal pixel along the lanes are
+//                     found with shfl_up + ballot and the run head issues ONE
+//                     atomicAdd(run length) (red.global.add.u32 resolved in L2).
+//   a6 scheduling     one tile per CTA, tiles aligned to the GLOBAL grid and rasterised
+//                     row-major so that concurrently resident CTAs touch a narrow band of
+//                     the map; rays outside the requested region are masked.
+//
+// Summation order and precision:
+//   lenses in index order; FP32 partial sums over groups of KF consecutive lenses (groups
+//   aligned to multiples of KF in lens index) are added, in order, to one fp64
+//   accumulator per ray and component.  With Real = double the partials are fp64 too
+//   and the reciprocal is an IEEE division.
+//   Every FP32 operation is written with an explicit-rounding intrinsic so that the
+//   compiler can neither contract nor reassociate: the arithmetic of a ray does not
+//   depend on the template instantiation (shoot vs capture) it runs in.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mlb200 {
+
+struct ShootParams {
+    const double2 *lens;      // [n_lens] fp64 (x, y), device
+    int n_lens;
+    int n_pix;
+    long long i0, i1, j0, j1; // region of ray indices to count (others are masked)
+    long long tile_i0, tile_j0; // first global tile index along each axis for this launch
+    long long tiles_x;        // tiles per row of this launch
+    long long tile_base;      // added to blockIdx.x (launches of > 2^31-1 tiles are split)
+    double delta;             // ray spacing
+    double half1, half2;      // (n1-1)/2, (n2-1)/2
+    double c1, c2;            // 1 - gamma - kappa_c, 1 + gamma - kappa_c
+    double halfL, inv_pixel;  // L/2, n_pix/L
+    unsigned int *map;        // [n_pix*n_pix] counts, device
+    unsigned long long *counters; // [0] shot [1] in map [2] dropped
+    double2 *capture;         // CAPTURE: [n_tiles_in_list * TW*TH] source-plane positions
+    const long long *tile_list; // CAPTURE: pairs (tile_i, tile_j), global tile indices
+};
+
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kChunk = 512; // lenses per shared-memory stage
+
+template <typename Real> struct Vec2;
+template <> struct Vec2<float> { using type = float2; };
+template <> struct Vec2<double> { using type = double2; };
+
+// A lens this far away contributes exactly zero: d^2 overflows to +inf, 1/inf = +0,
+// d * 0 = 0 (d itself stays finite).  Used to pad the last chunk to a multiple of 8.
+template <typename Real, bool NEWTON> __device__ __forceinline__ Real pad_coordinate();
+template <> __device__ __forceinline__ float pad_coordinate<float, false>() { return 1e30f; }
+// with the Newton step inf * 0 would give NaN: stay finite (term ~ 5e-19, below every rounding)
+template <> __device__ __forceinline__ float pad_coordinate<float, true>() { return 1e18f; }
+template <> __device__ __forceinline__ double pad_coordinate<double, false>() { return 1e200; }
+template <> __device__ __forceinline__ double pad_coordinate<double, true>() { return 1e200; }
+
+__device__ __forceinline__ float rcp_approx(float a)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); // one MUFU.RCP
+    return r;
+}
+
+template <bool NEWTON> __device__ __forceinline__ float recip(float a)
+{
+    float r = rcp_approx(a);
+    if (NEWTON) { // one Newton-Raphson step removes the approximation's error to < 1 ulp
+        float e = __fmaf_rn(-a, r, 1.0f);
+        r = __fmaf_rn(r, e, r);
+    }
+    return r;
+}
+template <bool NEWTON> __device__ __forceinline__ double recip(double a) { return 1.0 / a; }
+
+__device__ __forceinline__ float sub_rn(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ double sub_rn(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float fma_rn(float a, float b, float c) { return __fmaf_rn(a, b, c); }
+__device__ __forceinline__ double fma_rn(double a, double b, double c) { return __fma_rn(a, b, c); }
+
+template <typename Real, int RX, int RY, int KF, bool NEWTON, bool CAPTURE>
+__global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
+{
+    using Real2 = typename Vec2<Real>::type;
+    constexpr int TW = 32 * RX;
+    constexpr int TH = kWarps * RY;
+    static_assert(kChunk % KF == 0 && KF % 8 == 0, "flush groups must tile a chunk");
+    static_assert(kChunk % kThreads == 0, "staging assumes whole lenses per thread");
+    constexpr int PER_THREAD = kChunk / kThreads;
+
+    __shared__ __align__(16) Real2 lens_s[2][kChunk];
+    __shared__ unsigned int cta_count[3];
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+
+    // ---- a6: which tile
+    long long ti, tj;
+    const long long t = (long long)blockIdx.x + p.tile_base;
+    if (CAPTURE) {
+        ti = p.tile_list[2 * t];
+        tj = p.tile_list[2 * t + 1];
+    } else {
+        ti = p.tile_i0 + t % p.tiles_x;
+        tj = p.tile_j0 + t / p.tiles_x;
+    }
+    if (threadIdx.x < 3) cta_count[threadIdx.x] = 0;
+
+    // ---- a2: tile centre (fp64) and this thread's ray offsets from it
+    const double cx = ((double)(ti * TW) + 0.5 * (TW - 1) - p.half1) * p.delta;
+    const double cy = ((double)(tj * TH) + 0.5 * (TH - 1) - p.half2) * p.delta;
+    Real ox[RX], oy[RY];
+#pragma unroll
+    for (int c = 0; c < RX; ++c) ox[c] = (Real)(((double)(lane * RX + c) - 0.5 * (TW - 1)) * p.delta);
+#pragma unroll
+    for (int r = 0; r < RY; ++r) oy[r] = (Real)(((double)(warp * RY + r) - 0.5 * (TH - 1)) * p.delta);
+
+    double Sx[RY][RX], Sy[RY][RX]; // fp64 accumulators of the deflection sum
+    Real sx[RY][RX], sy[RY][RX];   // partial sums of the current flush group
+#pragma unroll
+    for (int r = 0; r < RY; ++r)
+#pragma unroll
+        for (int c = 0; c < RX; ++c) {
+            Sx[r][c] = 0.0; Sy[r][c] = 0.0;
+            sx[r][c] = (Real)0; sy[r][c] = (Real)0;
+        }
+
+    // ---- a1: stage chunk 0
+    const Real pad = pad_coordinate<Real, NEWTON>();
+    double2 pre[PER_THREAD];
+    auto fetch = [&](int base) {
+#pragma unroll
+        for (int q = 0; q < PER_THREAD; ++q) {
+            const int k = base + q * kThreads + threadIdx.x;
+            if (k < p.n_lens) pre[q] = __ldg(&p.lens[k]);
+        }
+    };
+    auto stage = [&](int base, int buf) {
+#pragma unroll
+        for (int q = 0; q < PER_THREAD; ++q) {
+            const int k = base + q * kThreads + threadIdx.x;
+            Real2 v;
+            if (k < p.n_lens) {
+                v.x = (Real)(pre[q].x - cx);
+                v.y = (Real)(pre[q].y - cy);
+            } else {
+                v.x = pad; v.y = pad;
+            }
+            lens_s[buf][q * kThreads + threadIdx.x] = v;
+        }
+    };
+    fetch(0);
+    stage(0, 0);
+    __syncthreads();
+
+    // ---- a3: all-pairs deflection sum
+    int buf = 0;
+    for (int base = 0; base < p.n_lens; base += kChunk) {
+        const bool more = base + kChunk < p.n_lens;
+        if (more) fetch(base + kChunk);
+        const int cnt = min(kChunk, p.n_lens - base);
+        const int cntp = (cnt + 7) & ~7; // padded with zero-contribution lenses
+        const Real2 *ls = lens_s[buf];
+        for (int k0 = 0; k0 < cntp; k0 += KF) {
+            const int kend = min(k0 + KF, cntp);
+#pragma unroll 1
+            for (int k = k0; k < kend; k += 2) {
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const Real2 l = ls[k + u];
+                    Real dx[RX], dx2[RX], dy[RY], dy2[RY];
+#pragma unroll
+                    for (int c = 0; c < RX; ++c) { dx[c] = sub_rn(ox[c], l.x); dx2[c] = mul_rn(dx[c], dx[c]); }
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) { dy[r] = sub_rn(oy[r], l.y); dy2[r] = mul_rn(dy[r], dy[r]); }
+#pragma unroll
+                    for (int r = 0; r < RY; ++r)
+#pragma unroll
+                        for (int c = 0; c < RX; ++c) {
+                            const Real inv = recip<NEWTON>(add_rn(dx2[c], dy2[r]));
+                            sx[r][c] = fma_rn(dx[c], inv, sx[r][c]);
+                            sy[r][c] = fma_rn(dy[r], inv, sy[r][c]);
+                        }
+                }
+            }
+            // flush the group's partial sums into the fp64 accumulators
+#pragma unroll
+            for (int r = 0; r < RY; ++r)
+#pragma unroll
+                for (int c = 0; c < RX; ++c) {
+                    Sx[r][c] += (double)sx[r][c]; sx[r][c] = (Real)0;
+                    Sy[r][c] += (double)sy[r][c]; sy[r][c] = (Real)0;
+                }
+        }
+        if (more) stage(base + kChunk, buf ^ 1);
+        __syncthreads();
+        buf ^= 1;
+    }
+
+    // ---- a4 + a5: macro terms, pixel, binning
+    unsigned int n_shot = 0, n_in = 0, n_drop = 0; // warp-uniform
+    const unsigned int full = 0xffffffffu;
+#pragma unroll
+    for (int r = 0; r < RY; ++r) {
+        const long long j = tj * TH + warp * RY + r;
+        const double x2 = ((double)j - p.half2) * p.delta;
+        const bool jvalid = (j >= p.j0) && (j < p.j1);
+#pragma unroll
+        for (int c = 0; c < RX; ++c) {
+            const long long i = ti * TW + lane * RX + c;
+            const double x1 = ((double)i - p.half1) * p.delta;
+            const double y1 = p.c1 * x1 - Sx[r][c];
+            const double y2 = p.c2 * x2 - Sy[r][c];
+            const bool finite = (fabs(y1) <= 1.7976931348623157e308) && (fabs(y2) <= 1.7976931348623157e308);
+            if (CAPTURE) {
+                const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+                double2 o;
+                o.x = finite ? y1 : qnan;
+                o.y = finite ? y2 : qnan;
+                p.capture[(size_t)t * (TW * TH) + (size_t)(warp * RY + r) * TW + lane * RX + c] = o;
+            } else {
+                const bool valid = jvalid && (i >= p.i0) && (i < p.i1);
+                const double u1 = (y1 + p.halfL) * p.inv_pixel;
+                const double u2 = (y2 + p.halfL) * p.inv_pixel;
+                const double np = (double)p.n_pix;
+                const bool inside = (u1 >= 0.0) && (u1 < np) && (u2 >= 0.0) && (u2 < np);
+                int pix = -1;
+                if (valid && finite && inside) pix = (int)u2 * p.n_pix + (int)u1;
+                // run-length aggregation along the lanes of the warp
+                const int prev = __shfl_up_sync(full, pix, 1);
+                const bool head = (lane == 0) || (pix != prev);
+                const unsigned int heads = __ballot_sync(full, head);
+                const unsigned int inmask = __ballot_sync(full, pix >= 0);
+                if (head && pix >= 0) {
+                    const unsigned int above = heads & ~((2u << lane) - 1u);
+                    const int next = above ? (__ffs(above) - 1) : 32;
+                    atomicAdd(&p.map[pix], (unsigned int)(next - lane));
+                }
+                n_in += __popc(inmask);
+                n_shot += __popc(__ballot_sync(full, valid));
+                n_drop += __popc(__ballot_sync(full, valid && !finite));
+            }
+        }
+    }
+    if (!CAPTURE) {
+        if (lane == 0) {
+            atomicAdd(&cta_count[0], n_shot);
+            atomicAdd(&cta_count[1], n_in);
+            if (n_drop) atomicAdd(&cta_count[2], n_drop);
+        }
+        __syncthreads();
+        if (threadIdx.x < 3 && cta_count[threadIdx.x])
+            atomicAdd(&p.counters[threadIdx.x], (unsigned long long)cta_count[threadIdx.x]);
+    }
+}
+
+} // namespace mlb200

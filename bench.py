@@ -1,0 +1,324 @@
+#!/usr/bin/env python
+"""bench.py -- lens-ray interactions/s of the fused shoot kernel on BASELINE.json:configs[1].
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2] [--impl reference]
+
+A step is one pass of the whole hot path (lens staging, fused ray
+generation, deflection sum, macro terms, binning; map zeroing included) over the full ray
+grid of the workload: one ml_shoot (N = 1) or one row band per rank plus the map all-reduce
+(N > 1, strong scaling).  Prints ONE JSON line (rank 0).  DESIGN.md "Measurement" explains
+every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from workloads import CONFIGS, lens_disk, parity_tiles  # noqa: E402
+
+METRIC = "lens-ray interactions/sec"
+UNIT = "interactions/s"
+N_FLOP = 10.0          # flop per lens-ray interaction
+FP32_LANES_PER_SM = 128
+
+
+def problem_args(p):
+    return (p.sigma, p.stellar_fraction, p.gamma, p.n_pix, p.n_rays, p.L)
+
+
+def pick(name):
+    for p in CONFIGS:
+        if p.name == name:
+            return p
+    raise SystemExit("unknown workload %r" % name)
+
+
+# ------------------------------------------------------------------ clocks (recipe: B200_PROFILING.md)
+class ClockSampler:
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            f = tempfile.NamedTemporaryFile("w", suffix=".csv", delete=False)
+            self.path = f.name
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                 "--format=csv,noheader,nounits", "-lms", "100"], stdout=f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        try:
+            for line in open(self.path):
+                c = [x.strip() for x in line.split(",")]
+                if len(c) < 9:
+                    continue
+                try:
+                    sm.append(float(c[1])); mx.append(float(c[2])); pw.append(float(c[3]))
+                except ValueError:
+                    continue
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm),
+                       power_w_max=float(max(pw)), sm_mhz_min=float(min(sm)), reasons=sorted(reasons))
+        return out
+
+
+# ------------------------------------------------------------------ oracle legs
+def oracle_rate(p, seconds, log=None):
+    """Time the fp64 CPU oracle, as it stands, on a bounded sample of workload p: seeded
+    512 x 512-ray sub-rectangles of its ray grid, as many as fit in about `seconds`."""
+    from oracle import oracle
+    g = oracle.geometry(*problem_args(p))
+    xy = lens_disk(g.n_star, g.r_star, p.seed)
+    side = 512
+    tiles = parity_tiles(g.n1, g.n2, 64, side, p.seed)
+    omap = np.zeros((p.n_pix, p.n_pix), dtype=np.uint32)
+    t0 = time.perf_counter()
+    oracle.shoot_region(*problem_args(p), xy, region=(0, 128, 0, 128), map_out=omap)  # calibrate
+    per_inter = (time.perf_counter() - t0) / (128 * 128 * max(g.n_star, 1))
+    n_tiles = int(max(1, min(len(tiles), seconds / (per_inter * side * side * max(g.n_star, 1)))))
+    omap[:] = 0
+    inter = 0
+    t0 = time.perf_counter()
+    for r in tiles[:n_tiles]:
+        _, st = oracle.shoot_region(*problem_args(p), xy, region=r, map_out=omap)
+        inter += st["interactions"]
+    dt = time.perf_counter() - t0
+    return {"value": inter / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": "%s: %d seeded sub-rectangles of %dx%d rays x %d lenses = %.3g interactions in %.1f s"
+                      % (p.name, n_tiles, side, side, g.n_star, inter, dt),
+            "seconds": dt, "interactions": inter}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric / unit / config."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    p = pick(args.workload)
+    per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_rate(p, per_step)
+    inter, secs, last = 0, 0.0, None
+    for _ in range(args.steps):
+        last = oracle_rate(p, per_step)
+        inter += last["interactions"]
+        secs += last["seconds"]
+    value = inter / secs
+    base = {"value": value, "unit": UNIT, "cores": last["cores"], "kind": "oracle", "sample": last["sample"] + " per step"}
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+            "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": config_dict(p, None, args),
+            "cpu_baseline": base,
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def config_dict(p, info, args):
+    c = {"workload": "%s: sigma=%g gamma=%g stellar_fraction=%g L=%g n_pix=%d^2 n_rays=%g seed=%d (BASELINE.json configs[%d])"
+                     % (p.name, p.sigma, p.gamma, p.stellar_fraction, p.L, p.n_pix, p.n_rays, p.seed, CONFIGS.index(p)),
+         "l2": "flushed between steps (256 MiB write)",
+         "parallelism": "ray row bands x%d + map all-reduce" % args.gpus if args.gpus > 1 else "single GPU"}
+    if info is not None:
+        c.update(n_lenses=int(info["n_lenses"]), n1=int(info["n1"]), n2=int(info["n2"]),
+                 rays=int(info["n1"]) * int(info["n2"]), tile=[int(info["tile_w"]), int(info["tile_h"])],
+                 precision=args.precision)
+    return c
+
+
+# ------------------------------------------------------------------ the CUDA arm
+PRECISIONS = {"fp32_tiled": 0, "fp32_compensated": 1, "fp64": 2}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1005_5198_b200 as ml
+    from paper_1005_5198_b200.sharding import allreduce_map, row_band
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; --impl reference times the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    assert world == args.gpus or world == 1, "launch with torchrun --nproc-per-node == --gpus"
+
+    p = pick(args.workload)
+    m = ml.MagnificationMap(*problem_args(p), device=local, precision=PRECISIONS[args.precision])
+    info = m.info
+    xy = lens_disk(info["n_star_expected"], info["r_star"], p.seed)
+    m.set_lenses(xy)
+    info = m.info
+    n1, n2, n_lens = int(info["n1"]), int(info["n2"]), int(info["n_lenses"])
+    j0, j1 = row_band(n2, rank, world, int(info["tile_h"]))
+
+    stream = torch.cuda.Stream(device=dev)
+    counts = torch.zeros((p.n_pix, p.n_pix), dtype=torch.int32, device=dev)  # torch owns the map memory
+    m.use_device_map(counts.data_ptr())
+    m.attach_stream(stream.cuda_stream)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    host_xy = torch.from_numpy(xy).pin_memory()
+    host_map = torch.empty((p.n_pix, p.n_pix), dtype=torch.int32).pin_memory()
+    host_map_np = host_map.numpy().view(np.uint32)
+
+    def step():
+        with torch.cuda.stream(stream):
+            flush.fill_(1)                       # evict L2 between steps
+            m.shoot_region(0, n1, j0, j1)        # zero map + fused kernel (synchronises `stream`)
+            st = m.stats
+            if world > 1:
+                allreduce_map(counts)
+        return st
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(args.warmup):
+        step()
+    sampler = ClockSampler(local)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kernel_ms, launches, rays = 0.0, 0, 0
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        st = step()
+        kernel_ms += st["kernel_ms"]
+        launches += int(st["kernel_launches"])
+        rays += int(st["rays_shot"])
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if rank == 0 else None
+    agg = torch.tensor([ms, kernel_ms], dtype=torch.float64, device=dev)
+    tot = torch.tensor([rays, launches], dtype=torch.int64, device=dev)
+    if world > 1:
+        dist.all_reduce(agg, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    ms, kernel_ms_max = float(agg[0]), float(agg[1])
+    rays_all, launches_all = int(tot[0]), int(tot[1])
+    assert rays_all == n1 * n2 * args.steps, (rays_all, n1 * n2 * args.steps)
+    value = rays_all * n_lens / (ms * 1e-3)
+
+    # ---- end to end through the public C ABI with HOST buffers, copies inside the timed region
+    e2e_steps = max(1, min(args.steps, 3))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        m.set_lenses(host_xy.numpy())            # H2D: lens positions (host buffer -> ml_set_lenses)
+        m.shoot_region(0, n1, j0, j1)
+        if world > 1:
+            with torch.cuda.stream(stream):
+                allreduce_map(counts)
+        m.counts(out=host_map_np)                # D2H: the map (ml_get_map -> host buffer)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    e2e_t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
+    e2e_value = n1 * n2 * n_lens * e2e_steps / float(e2e_t[0])
+    m.close()
+    if world > 1:
+        dist.destroy_process_group()
+    if rank != 0:
+        return 0
+
+    sm_count = int(info["sm_count"])
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    max_mhz = float(peaks.get("sm_max_mhz") or (info["sm_clock_khz"] / 1e3))
+    peak_tflops = sm_count * FP32_LANES_PER_SM * 2 * max_mhz * 1e6 / 1e12
+    kernel_s_per_launch = kernel_ms_max * 1e-3 / max(1, launches_all // max(world, 1))
+    inter_per_launch = (rays_all // world) * n_lens / max(1, launches_all // max(world, 1))
+    achieved = N_FLOP * inter_per_launch / kernel_s_per_launch / 1e12
+    roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": achieved / peak_tflops, "traffic": None,
+                "note": "nominal %g flop/interaction (PAPER.md:66); peak = %d SMs x 128 FP32 lanes x 2 x %.0f MHz "
+                        "(MEASURED_PEAKS.json sm_max_mhz); kernel time = CUDA events on the launching stream"
+                        % (N_FLOP, sm_count, max_mhz),
+                "kernel_ms_per_launch": 1e3 * kernel_s_per_launch}
+    if clocks and clocks.get("sm_mhz"):
+        roofline["frac_at_sampled_clock"] = achieved / (peak_tflops * clocks["sm_mhz"] / max_mhz)
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu = oracle_rate(p, args.cpu_seconds)
+        cpu = {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "strong", "vs_baseline": None, "dtype": "f32" if args.precision != "fp64" else "f64",
+            "data": "synthetic", "config": config_dict(p, info, args),
+            "rays_per_s": rays_all / (ms * 1e-3), "map_wall_ms": ms / args.steps,
+            "nominal_tflops": N_FLOP * value / 1e12, "frac_fp32_peak": N_FLOP * value / 1e12 / (peak_tflops * args.gpus),
+            "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(xy.nbytes),
+                    "d2h_bytes_per_step": int(host_map_np.nbytes + 24), "steps": e2e_steps},
+            "gpu_launches": launches_all}
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C2", help="C1..C5 (BASELINE.json configs); the metric is quoted on C2")
+    ap.add_argument("--precision", default="fp32_tiled", choices=sorted(PRECISIONS))
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        print("bench.py: note: --warmup < 3 breaks the timing rules", file=sys.stderr)
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

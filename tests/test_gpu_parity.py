@@ -1,0 +1,105 @@
+"""-m gpu parity tests: the CUDA library, called through its C ABI, against the fp64 CPU
+oracle on the same seeded inputs (BASELINE.json:north_star criteria):
+
+  1. source-plane positions of sampled rays within 1e-3 pixel widths,
+  2. >= 99.99 % of rays in the oracle's pixel,
+  3. total in-map counts within 1e-5 relative,
+  4. |mu_gpu - mu_oracle| <= 1e-3 on 8x8-block averages,
+
+on C1 whole, on seeded sub-regions of C2-C5 (the oracle would need hours for their full
+maps: SURVEY.md section 8(c) "parity ladder"), and at C2's full size
+in the launch configuration bench.py times (sampled rays + invariants).
+"""
+import numpy as np
+import pytest
+
+import paper_1005_5198_b200 as ml
+from oracle import oracle
+from workloads import CONFIGS, lens_disk, probe_rays
+
+from parity_common import (check_maps, check_rays, make_pair, problem_args, subregion_tiles)
+
+pytestmark = pytest.mark.gpu
+
+PRECISIONS = [ml.ML_PREC_FP32_TILED, ml.ML_PREC_FP32_COMPENSATED, ml.ML_PREC_FP64]
+PREC_IDS = ["fp32_tiled", "fp32_compensated", "fp64"]
+
+
+@pytest.mark.parametrize("precision", PRECISIONS, ids=PREC_IDS)
+def test_c1_whole_map_all_four_criteria(precision):
+    p = CONFIGS[0]
+    m, g, xy = make_pair(p, precision)
+    with m:
+        m.shoot()
+        gmap, gst = m.counts(), m.stats
+        omap, ost = oracle.shoot(*problem_args(p), xy)
+        # golden integers of the C1 worked example (oracle side; SURVEY.md 8(c) pin (e))
+        assert ost["rays_shot"] == 6553600 and ost["rays_in_map"] == 4012112
+        r = check_maps(p, gmap, gst, omap, ost)
+        y_g = m.capture_region(0, g.n1, 0, g.n2)
+        y_o = oracle.capture_region(*problem_args(p), xy, (0, g.n1, 0, g.n2))
+        r.update(check_rays(p, g, y_g, y_o))
+        # the shoot and capture instantiations run the same arithmetic: binning the
+        # captured positions (oracle's floor rule) reproduces the device map exactly
+        pix = oracle.pixels_of(*problem_args(p), y_g).ravel()
+        rebinned = np.bincount(pix[pix >= 0], minlength=p.n_pix * p.n_pix).reshape(p.n_pix, p.n_pix)
+        assert np.array_equal(rebinned, gmap)
+        if precision == ml.ML_PREC_FP64:
+            assert r["same_pixel"] >= 0.999999
+        print("C1", PREC_IDS[PRECISIONS.index(precision)], r)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4], ids=["C2", "C3", "C4", "C5"])
+@pytest.mark.parametrize("precision", [ml.ML_PREC_FP32_TILED, ml.ML_PREC_FP64], ids=["fp32_tiled", "fp64"])
+def test_subregions_all_four_criteria(cfg, precision):
+    p = CONFIGS[cfg]
+    m, g, xy = make_pair(p, precision)
+    with m:
+        tiles = subregion_tiles(p, g, xy.shape[0])
+        omap = np.zeros((p.n_pix, p.n_pix), dtype=np.uint32)
+        ost = {"rays_shot": 0, "rays_in_map": 0}
+        same_w, rays, pos = 0.0, 0, 0.0
+        for t, (i0, i1, j0, j1) in enumerate(tiles):
+            m.shoot_region(i0, i1, j0, j1, accumulate=(t > 0))
+            _, st = oracle.shoot_region(*problem_args(p), xy, region=(i0, i1, j0, j1), map_out=omap)
+            for k in ost:
+                ost[k] += st[k]
+        r = check_maps(p, m.counts(), m.stats, omap, ost)
+        # per-ray criteria on every ray of the first tiles (capture = same kernel arithmetic)
+        for (i0, i1, j0, j1) in tiles[:4]:
+            y_g = m.capture_region(i0, i1, j0, j1)
+            y_o = oracle.capture_region(*problem_args(p), xy, (i0, i1, j0, j1))
+            rr = check_rays(p, g, y_g, y_o)
+            same_w += rr["same_pixel"] * rr["rays"]
+            rays += rr["rays"]
+            pos = max(pos, rr["pos_err_pixels"])
+        r.update(same_pixel=same_w / rays, pos_err_pixels=pos, rays=rays, tiles=len(tiles))
+        print(p.name, r)
+
+
+def test_c2_full_size_bench_configuration():
+    """C2 whole (8.4e9 rays), exactly what bench.py launches: invariants that hold at any
+    size plus sampled rays the oracle computes one by one."""
+    p = CONFIGS[1]
+    m, g, xy = make_pair(p)
+    with m:
+        m.shoot()
+        st, gmap = m.stats, m.counts()
+        assert st["rays_shot"] == g.n1 * g.n2
+        assert st["interactions"] == g.n1 * g.n2 * xy.shape[0]
+        assert int(gmap.sum(dtype=np.uint64)) == st["rays_in_map"]
+        assert st["rays_dropped"] == 0
+        # mean magnification within the sanity band of SURVEY.md 8(c) pin (d)
+        ratio = gmap.mean() / p.n_rays / abs(g.mu_th)
+        assert 0.88 <= ratio <= 1.12, ratio
+        ri, rj = probe_rays(g.n1, g.n2, 200000, p.seed)
+        y_g = m.probe(ri, rj)
+        y_o = oracle.probe(*problem_args(p), xy, ri, rj)
+        r = check_rays(p, g, y_g, y_o)
+        # a sub-rectangle shot alone equals its share of the full run bit for bit: compare
+        # the oracle's partial map with the device's on the same region
+        i0, i1, j0, j1 = 40000, 40700, 50000, 50900
+        m.shoot_region(i0, i1, j0, j1)
+        omap, ost = oracle.shoot_region(*problem_args(p), xy, region=(i0, i1, j0, j1))
+        r.update(check_maps(p, m.counts(), m.stats, omap, ost))
+        print("C2 full", r, "mean ratio", ratio)

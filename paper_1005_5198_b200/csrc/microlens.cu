@@ -56,13 +56,15 @@ struct DeviceGuard {
 struct Mode {
     int tw, th;
 };
-constexpr int RXF = 4, RYF = 4, KFF = 64;  // FP32_TILED
+constexpr int RXF = 4, RYF = 4, KFF = 64;  // FP32_TILED (shoot_kernel_pipe) and FP32_COMPENSATED
+constexpr int WARPS_T = 4, SHARED_T = 4, MINB_T = 3; // FP32_TILED: 128-thread CTAs, 3 per SM, all rows share
 constexpr int KFC = 8;                     // FP32_COMPENSATED
 constexpr int RXD = 2, RYD = 2, KFD = 64;  // FP64
 
 Mode mode_of(int precision)
 {
     if (precision == ML_PREC_FP64) return {32 * RXD, kWarps * RYD};
+    if (precision == ML_PREC_FP32_TILED) return {32 * RXF, WARPS_T * RYF};
     return {32 * RXF, kWarps * RYF};
 }
 
@@ -78,7 +80,7 @@ template <bool CAPTURE> cudaError_t launch(int precision, long long n_tiles, con
         shoot_kernel<float, RXF, RYF, KFC, true, CAPTURE><<<g, kThreads, 0, s>>>(p);
         break;
     default:
-        shoot_kernel<float, RXF, RYF, KFF, false, CAPTURE><<<g, kThreads, 0, s>>>(p);
+        shoot_kernel_pipe<SHARED_T, KFF, WARPS_T, MINB_T, true, CAPTURE><<<g, WARPS_T * 32, 0, s>>>(p);
         break;
     }
     return cudaGetLastError();

@@ -98,6 +98,72 @@ __device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(
 __device__ __forceinline__ float fma_rn(float a, float b, float c) { return __fmaf_rn(a, b, c); }
 __device__ __forceinline__ double fma_rn(double a, double b, double c) { return __fma_rn(a, b, c); }
 
+// a4 + a5 (+ statistics) for one thread's RX x RY rays: macro terms and pixel index in
+// fp64, run-length aggregated binning.  Shared by every instantiation of the kernels below.
+template <int RX, int RY, bool CAPTURE, int WARPS = kWarps>
+__device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, long long tj, long long t, int lane,
+                                            int warp, const double (&Sx)[RY][RX], const double (&Sy)[RY][RX],
+                                            unsigned int *cta_count)
+{
+    constexpr int TW = 32 * RX;
+    constexpr int TH = WARPS * RY;
+    // ---- a4 + a5: macro terms, pixel, binning
+    unsigned int n_shot = 0, n_in = 0, n_drop = 0; // warp-uniform
+    const unsigned int full = 0xffffffffu;
+#pragma unroll
+    for (int r = 0; r < RY; ++r) {
+        const long long j = tj * TH + warp * RY + r;
+        const double x2 = ((double)j - p.half2) * p.delta;
+        const bool jvalid = (j >= p.j0) && (j < p.j1);
+#pragma unroll
+        for (int c = 0; c < RX; ++c) {
+            const long long i = ti * TW + lane * RX + c;
+            const double x1 = ((double)i - p.half1) * p.delta;
+            const double y1 = p.c1 * x1 - Sx[r][c];
+            const double y2 = p.c2 * x2 - Sy[r][c];
+            const bool finite = (fabs(y1) <= 1.7976931348623157e308) && (fabs(y2) <= 1.7976931348623157e308);
+            if (CAPTURE) {
+                const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+                double2 o;
+                o.x = finite ? y1 : qnan;
+                o.y = finite ? y2 : qnan;
+                p.capture[(size_t)t * (TW * TH) + (size_t)(warp * RY + r) * TW + lane * RX + c] = o;
+            } else {
+                const bool valid = jvalid && (i >= p.i0) && (i < p.i1);
+                const double u1 = (y1 + p.halfL) * p.inv_pixel;
+                const double u2 = (y2 + p.halfL) * p.inv_pixel;
+                const double np = (double)p.n_pix;
+                const bool inside = (u1 >= 0.0) && (u1 < np) && (u2 >= 0.0) && (u2 < np);
+                int pix = -1;
+                if (valid && finite && inside) pix = (int)u2 * p.n_pix + (int)u1;
+                // run-length aggregation along the lanes of the warp
+                const int prev = __shfl_up_sync(full, pix, 1);
+                const bool head = (lane == 0) || (pix != prev);
+                const unsigned int heads = __ballot_sync(full, head);
+                const unsigned int inmask = __ballot_sync(full, pix >= 0);
+                if (head && pix >= 0) {
+                    const unsigned int above = heads & ~((2u << lane) - 1u);
+                    const int next = above ? (__ffs(above) - 1) : 32;
+                    atomicAdd(&p.map[pix], (unsigned int)(next - lane));
+                }
+                n_in += __popc(inmask);
+                n_shot += __popc(__ballot_sync(full, valid));
+                n_drop += __popc(__ballot_sync(full, valid && !finite));
+            }
+        }
+    }
+    if (!CAPTURE) {
+        if (lane == 0) {
+            atomicAdd(&cta_count[0], n_shot);
+            atomicAdd(&cta_count[1], n_in);
+            if (n_drop) atomicAdd(&cta_count[2], n_drop);
+        }
+        __syncthreads();
+        if (threadIdx.x < 3 && cta_count[threadIdx.x])
+            atomicAdd(&p.counters[threadIdx.x], (unsigned long long)cta_count[threadIdx.x]);
+    }
+}
+
 template <typename Real, int RX, int RY, int KF, bool NEWTON, bool CAPTURE>
 __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
 {
@@ -217,61 +283,193 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
         buf ^= 1;
     }
 
-    // ---- a4 + a5: macro terms, pixel, binning
-    unsigned int n_shot = 0, n_in = 0, n_drop = 0; // warp-uniform
-    const unsigned int full = 0xffffffffu;
+    finish_tile<RX, RY, CAPTURE>(p, ti, tj, t, lane, warp, Sx, Sy, cta_count);
+}
+
+// ---------------------------------------------------------------------------------------
+// The default FP32 kernel (ML_PREC_FP32_TILED): packed f32x2 arithmetic, shared reciprocals,
+// software-pipelined over lenses.
+//
+// The generic kernel above issues one MUFU.RCP per interaction, and the special-function unit
+// (16 results per clock per SM) caps it at 62.5 % of the FP32 peak in the paper's 10-flop
+// accounting.  Here a thread still owns 4 x 4 rays, but
+//   * every FP32 instruction on the rays is a packed FADD2 / FMUL2 / FFMA2 on two rays that are
+//     adjacent along axis 1 (columns 0,1 = "A", columns 2,3 = "B"): half the issue slots, so the
+//     MUFU instructions issue beside a busy FMA pipe;
+//   * on SHARED of the 4 rows one reciprocal serves two interactions:
+//         R = 1/(r2A * r2B),   1/r2A = R * r2B,   1/r2B = R * r2A      (3 FMUL2, 2 MUFU per 4)
+//     instead of 4 MUFU.  SHARED = 4: 40 packed + 4 scalar FP32 instructions and 8 MUFU per lens
+//     per thread (16 interactions) = 5.25 FMA-pipe lane-cycles and 0.5 MUFU per interaction;
+//   * the lens tile is staged as float4 (-x, -x, -y, -y): one LDS.128 broadcast per lens feeds
+//     the packed subtractions without any register shuffling;
+//   * stage 1 (differences, r^2, products, MUFU) of lens k+1 is issued before stage 2
+//     (1/r^2 = R * r2, the four accumulating FFMA2 per row) of lens k, so that no instruction
+//     waits on a reciprocal it has just issued (PipeRegs carries a lens between the stages).
+// r^2 = dy*dy + (dx*dx + 2^-80): the 2^-80 keeps a ray that coincides with a lens in its
+// FP32 tile-local coordinates from producing 0 * inf = NaN in its partner's term (the lens
+// is then simply not seen by that one ray, R12); it is below half an ulp of r^2 for
+// every ray that ends closer than 1e8 R_E to the map.
+// Summation order: as above (lens index order, groups of KF, fp64 accumulators).  A padding
+// lens sits at 1e15: r^2 = 2e30 stays finite, the shared product overflows to +inf, 1/inf = +0,
+// so its terms are exactly 0 on shared rows and 5e-16 on the others.
+template <int RY> struct PipeRegs {
+    float2 dxA, dxB;
+    float dy[RY];
+    float2 r2A[RY], r2B[RY]; // shared rows: r^2; other rows: 1/r^2
+    float2 R[RY];
+};
+
+template <int SHARED, int KF, int WARPS, int MINB, bool SCALAR_DY, bool CAPTURE>
+__global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const ShootParams p)
+{
+    constexpr int RX = 4, RY = 4;
+    constexpr int THREADS = WARPS * 32;
+    constexpr int TW = 32 * RX;
+    constexpr int TH = WARPS * RY;
+    static_assert(kChunk % KF == 0 && KF % 2 == 0, "flush groups must tile a chunk");
+    constexpr int PER_THREAD = kChunk / THREADS;
+
+    __shared__ __align__(16) float4 lens_s[2][kChunk + 2];
+    __shared__ unsigned int cta_count[3];
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+
+    long long ti, tj;
+    const long long t = (long long)blockIdx.x + p.tile_base;
+    if (CAPTURE) {
+        ti = p.tile_list[2 * t];
+        tj = p.tile_list[2 * t + 1];
+    } else {
+        ti = p.tile_i0 + t % p.tiles_x;
+        tj = p.tile_j0 + t / p.tiles_x;
+    }
+    if (threadIdx.x < 3) cta_count[threadIdx.x] = 0;
+    if (threadIdx.x < 4) lens_s[threadIdx.x >> 1][kChunk + (threadIdx.x & 1)] = make_float4(-1e15f, -1e15f, -1e15f, -1e15f);
+
+    const double cx = ((double)(ti * TW) + 0.5 * (TW - 1) - p.half1) * p.delta;
+    const double cy = ((double)(tj * TH) + 0.5 * (TH - 1) - p.half2) * p.delta;
+    float2 oxA, oxB;
+    float oy[RY];
+    oxA.x = (float)(((double)(lane * RX + 0) - 0.5 * (TW - 1)) * p.delta);
+    oxA.y = (float)(((double)(lane * RX + 1) - 0.5 * (TW - 1)) * p.delta);
+    oxB.x = (float)(((double)(lane * RX + 2) - 0.5 * (TW - 1)) * p.delta);
+    oxB.y = (float)(((double)(lane * RX + 3) - 0.5 * (TW - 1)) * p.delta);
+#pragma unroll
+    for (int r = 0; r < RY; ++r) oy[r] = (float)(((double)(warp * RY + r) - 0.5 * (TH - 1)) * p.delta);
+
+    double Sx[RY][RX], Sy[RY][RX];
+    float2 sxA[RY], sxB[RY], syA[RY], syB[RY];
 #pragma unroll
     for (int r = 0; r < RY; ++r) {
-        const long long j = tj * TH + warp * RY + r;
-        const double x2 = ((double)j - p.half2) * p.delta;
-        const bool jvalid = (j >= p.j0) && (j < p.j1);
 #pragma unroll
-        for (int c = 0; c < RX; ++c) {
-            const long long i = ti * TW + lane * RX + c;
-            const double x1 = ((double)i - p.half1) * p.delta;
-            const double y1 = p.c1 * x1 - Sx[r][c];
-            const double y2 = p.c2 * x2 - Sy[r][c];
-            const bool finite = (fabs(y1) <= 1.7976931348623157e308) && (fabs(y2) <= 1.7976931348623157e308);
-            if (CAPTURE) {
-                const double qnan = __longlong_as_double(0x7ff8000000000000LL);
-                double2 o;
-                o.x = finite ? y1 : qnan;
-                o.y = finite ? y2 : qnan;
-                p.capture[(size_t)t * (TW * TH) + (size_t)(warp * RY + r) * TW + lane * RX + c] = o;
+        for (int c = 0; c < RX; ++c) { Sx[r][c] = 0.0; Sy[r][c] = 0.0; }
+        sxA[r] = make_float2(0.f, 0.f); sxB[r] = sxA[r]; syA[r] = sxA[r]; syB[r] = sxA[r];
+    }
+
+    double2 pre[PER_THREAD];
+    auto fetch = [&](int base) {
+#pragma unroll
+        for (int q = 0; q < PER_THREAD; ++q) {
+            const int k = base + q * THREADS + threadIdx.x;
+            if (k < p.n_lens) pre[q] = __ldg(&p.lens[k]);
+        }
+    };
+    auto stage = [&](int base, int buf) {
+#pragma unroll
+        for (int q = 0; q < PER_THREAD; ++q) {
+            const int k = base + q * THREADS + threadIdx.x;
+            float nx = -1e15f, ny = -1e15f;
+            if (k < p.n_lens) {
+                nx = -(float)(pre[q].x - cx);
+                ny = -(float)(pre[q].y - cy);
+            }
+            lens_s[buf][q * THREADS + threadIdx.x] = make_float4(nx, nx, ny, ny);
+        }
+    };
+    fetch(0);
+    stage(0, 0);
+    __syncthreads();
+
+    const float2 eps2 = make_float2(0x1p-80f, 0x1p-80f);
+    auto stage1 = [&](const float4 l, PipeRegs<RY> &s) {
+        const float2 nlx = make_float2(l.x, l.y), nly = make_float2(l.z, l.w);
+        s.dxA = __fadd2_rn(oxA, nlx);
+        s.dxB = __fadd2_rn(oxB, nlx);
+        const float2 qA = __ffma2_rn(s.dxA, s.dxA, eps2), qB = __ffma2_rn(s.dxB, s.dxB, eps2);
+#pragma unroll
+        for (int r = 0; r < RY; ++r) {
+            float2 dy;
+            if (SCALAR_DY) {
+                s.dy[r] = __fadd_rn(oy[r], l.z);
+                dy = make_float2(s.dy[r], s.dy[r]);
             } else {
-                const bool valid = jvalid && (i >= p.i0) && (i < p.i1);
-                const double u1 = (y1 + p.halfL) * p.inv_pixel;
-                const double u2 = (y2 + p.halfL) * p.inv_pixel;
-                const double np = (double)p.n_pix;
-                const bool inside = (u1 >= 0.0) && (u1 < np) && (u2 >= 0.0) && (u2 < np);
-                int pix = -1;
-                if (valid && finite && inside) pix = (int)u2 * p.n_pix + (int)u1;
-                // run-length aggregation along the lanes of the warp
-                const int prev = __shfl_up_sync(full, pix, 1);
-                const bool head = (lane == 0) || (pix != prev);
-                const unsigned int heads = __ballot_sync(full, head);
-                const unsigned int inmask = __ballot_sync(full, pix >= 0);
-                if (head && pix >= 0) {
-                    const unsigned int above = heads & ~((2u << lane) - 1u);
-                    const int next = above ? (__ffs(above) - 1) : 32;
-                    atomicAdd(&p.map[pix], (unsigned int)(next - lane));
-                }
-                n_in += __popc(inmask);
-                n_shot += __popc(__ballot_sync(full, valid));
-                n_drop += __popc(__ballot_sync(full, valid && !finite));
+                dy = __fadd2_rn(make_float2(oy[r], oy[r]), nly);
+                s.dy[r] = dy.x;
+            }
+            s.r2A[r] = __ffma2_rn(dy, dy, qA);
+            s.r2B[r] = __ffma2_rn(dy, dy, qB);
+            if (r < SHARED) {
+                const float2 P = __fmul2_rn(s.r2A[r], s.r2B[r]);
+                s.R[r].x = rcp_approx(P.x);
+                s.R[r].y = rcp_approx(P.y);
+            } else {
+                s.r2A[r].x = rcp_approx(s.r2A[r].x); s.r2A[r].y = rcp_approx(s.r2A[r].y);
+                s.r2B[r].x = rcp_approx(s.r2B[r].x); s.r2B[r].y = rcp_approx(s.r2B[r].y);
             }
         }
-    }
-    if (!CAPTURE) {
-        if (lane == 0) {
-            atomicAdd(&cta_count[0], n_shot);
-            atomicAdd(&cta_count[1], n_in);
-            if (n_drop) atomicAdd(&cta_count[2], n_drop);
+    };
+    auto stage2 = [&](const PipeRegs<RY> &s) {
+#pragma unroll
+        for (int r = 0; r < RY; ++r) {
+            float2 iA, iB;
+            if (r < SHARED) {
+                iA = __fmul2_rn(s.R[r], s.r2B[r]);
+                iB = __fmul2_rn(s.R[r], s.r2A[r]);
+            } else {
+                iA = s.r2A[r];
+                iB = s.r2B[r];
+            }
+            const float2 dy = make_float2(s.dy[r], s.dy[r]);
+            sxA[r] = __ffma2_rn(s.dxA, iA, sxA[r]);
+            sxB[r] = __ffma2_rn(s.dxB, iB, sxB[r]);
+            syA[r] = __ffma2_rn(dy, iA, syA[r]);
+            syB[r] = __ffma2_rn(dy, iB, syB[r]);
         }
+    };
+
+    int buf = 0;
+    for (int base = 0; base < p.n_lens; base += kChunk) {
+        const bool more = base + kChunk < p.n_lens;
+        if (more) fetch(base + kChunk);
+        const int cnt = min(kChunk, p.n_lens - base);
+        const int cntp = (cnt + 1) & ~1;
+        const float4 *ls = lens_s[buf];
+        PipeRegs<RY> a, b;
+        stage1(ls[0], a);
+        for (int k0 = 0; k0 < cntp; k0 += KF) {
+            const int kend = min(k0 + KF, cntp);
+#pragma unroll 1
+            for (int k = k0; k < kend; k += 2) {
+                stage1(ls[k + 1], b);
+                stage2(a);
+                stage1(ls[k + 2], a);
+                stage2(b);
+            }
+#pragma unroll
+            for (int r = 0; r < RY; ++r) {
+                Sx[r][0] += (double)sxA[r].x; Sx[r][1] += (double)sxA[r].y;
+                Sx[r][2] += (double)sxB[r].x; Sx[r][3] += (double)sxB[r].y;
+                Sy[r][0] += (double)syA[r].x; Sy[r][1] += (double)syA[r].y;
+                Sy[r][2] += (double)syB[r].x; Sy[r][3] += (double)syB[r].y;
+                sxA[r] = make_float2(0.f, 0.f); sxB[r] = sxA[r]; syA[r] = sxA[r]; syB[r] = sxA[r];
+            }
+        }
+        if (more) stage(base + kChunk, buf ^ 1);
         __syncthreads();
-        if (threadIdx.x < 3 && cta_count[threadIdx.x])
-            atomicAdd(&p.counters[threadIdx.x], (unsigned long long)cta_count[threadIdx.x]);
+        buf ^= 1;
     }
+    finish_tile<RX, RY, CAPTURE, WARPS>(p, ti, tj, t, lane, warp, Sx, Sy, cta_count);
 }
 
 } // namespace mlb200

@@ -31,6 +31,11 @@ METRIC = "lens-ray interactions/sec"
 UNIT = "interactions/s"
 N_FLOP = 10.0          # flop per lens-ray interaction
 FP32_LANES_PER_SM = 128
+# DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel, from the
+# committed `ncu --set full` capture of this very command; None where no capture exists.
+NCU_DRAM_BYTES_PER_LAUNCH = {
+    ("C2", "fp32_tiled"): (4451584 + 0, "profiles/r01_ncu_full_c2_v2.txt"),
+}
 
 
 def problem_args(p):
@@ -279,7 +284,12 @@ def run_ours(args):
     inter_per_launch = (rays_all // world) * n_lens / max(1, launches_all // max(world, 1))
     achieved = N_FLOP * inter_per_launch / kernel_s_per_launch / 1e12
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops, "traffic": None,
+                "frac": achieved / peak_tflops,
+                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((p.name, args.precision), (None, None))[0] if world == 1 else None,
+                "traffic_unit": "bytes of DRAM traffic per launch (ncu --set full; %s); algorithmic HBM bytes per "
+                                "launch = n_pix^2*4 map + 16*N* lenses = %d"
+                                % (NCU_DRAM_BYTES_PER_LAUNCH.get((p.name, args.precision), (None, "no capture"))[1],
+                                   p.n_pix * p.n_pix * 4 + 16 * n_lens),
                 "note": "nominal %g flop/interaction (PAPER.md:66); peak = %d SMs x 128 FP32 lanes x 2 x %.0f MHz "
                         "(MEASURED_PEAKS.json sm_max_mhz); kernel time = CUDA events on the launching stream"
                         % (N_FLOP, sm_count, max_mhz),

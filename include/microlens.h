@@ -163,6 +163,51 @@ int ml_capture_region(ml_ctx *ctx, int64_t i0, int64_t i1, int64_t j0, int64_t j
  * Cost: one whole tile per distinct tile touched. */
 int ml_probe(ml_ctx *ctx, int64_t n, const int64_t *ray_i, const int64_t *ray_j, double *y_out);
 
+/* ---------------------------------------------------------------------------------------
+ * Map comparison (section 3.1): the paper's two accuracy measures between
+ * magnification maps -- the root-mean-square difference in magnitudes and a two-sample
+ * Kolmogorov-Smirnov test on the distributions of
+ *       Delta m_ij = -2.5 log10(mu_ij),   mu_ij = N_ij / N_rays        (eq. 10 :171, eq. 3 :47)
+ * computed on the device from two count maps (fp64 arithmetic, one fused pass over both
+ * maps plus small scans, readings M1-M4).
+ * --------------------------------------------------------------------------------------- */
+enum {
+    ML_MEM_HOST = 0,  /* the map pointers are HOST memory (copied to the device inside the call) */
+    ML_MEM_DEVICE = 1 /* the map pointers are DEVICE memory on `device` (e.g. ml_get_map_device)  */
+};
+
+typedef struct {
+    uint64_t n_pixels;             /* n                                                          */
+    uint64_t n_valid;              /* pixels with a count > 0 in BOTH maps (enter the RMS, M1)   */
+    uint64_t n_empty_a, n_empty_b; /* pixels with count 0                                        */
+    uint64_t sum_a, sum_b;         /* total counts                                               */
+    uint32_t max_a, max_b;         /* largest count                                              */
+    double mean_mu_a, mean_mu_b;   /* sum / (n * n_rays)  (eq. 3; compare with eq. 12)           */
+    double rms_delta_m;            /* sqrt(mean over the n_valid pixels of (dm_a - dm_b)^2), mag */
+    double ks_d;                   /* sup_x |F_a(x) - F_b(x)| over the Delta m of ALL pixels (an
+                                      empty pixel is a sample at +inf, M2)                       */
+    double ks_prob;                /* Q_KS((sqrt(Ne)+0.12+0.11/sqrt(Ne)) ks_d), Ne = n/2 (M3):
+                                      probability of a distance >= ks_d under the null hypothesis */
+    double kernel_ms;              /* device time of the kernels, CUDA events on the stream      */
+} ml_map_compare_result;
+
+/* Compare two count maps of n pixels each (same layout; n >= 1).  a, b: uint32 counts in HOST or
+ * DEVICE memory according to `where`; n_rays_a, n_rays_b > 0 are the maps' N_rays.  `cuda_stream`
+ * (cudaStream_t as void*, NULL = default stream) is used for all work; the call synchronises it.
+ * out = HOST struct.  K-S ties between the two maps are decided exactly when n_rays_a, n_rays_b
+ * have <= 26 significant bits.  ML_ERR_INVALID_ARG for NULL pointers, n < 1, n > 2^31-1,
+ * non-positive or non-finite n_rays, or a bad `where`; ML_ERR_OOM if a count >= 2^27 makes the
+ * count histogram too large; ML_ERR_CUDA without a device. */
+int ml_map_compare(const uint32_t *a, double n_rays_a, const uint32_t *b, double n_rays_b, int64_t n,
+                   int where, int32_t device, void *cuda_stream, ml_map_compare_result *out);
+
+/* Histogram of Delta m of one map (the "probability distribution for change in magnitude" of
+ * PAPER.md:169): hist_out[k] (HOST, n_bins uint64) = number of pixels with count > 0 and
+ * lo + k w <= Delta m < lo + (k+1) w, w = (hi-lo)/n_bins (half-open bins, M4); pixels outside
+ * [lo, hi) and empty pixels are not counted.  ML_ERR_INVALID_ARG unless lo < hi, 1 <= n_bins <= 2^20. */
+int ml_delta_m_histogram(const uint32_t *counts, double n_rays, int64_t n, double lo, double hi,
+                         int32_t n_bins, int where, int32_t device, void *cuda_stream, uint64_t *hist_out);
+
 /* Static description of a return code. */
 const char *ml_strerror(int code);
 

@@ -66,15 +66,20 @@ def ks_statistic(counts_a, n_rays_a, counts_b, n_rays_b):
     return float(np.abs(fa - fb).max()) if pts.size else 0.0
 
 
-def ks_probability(d, na, nb, terms=100):
-    """Q_KS: probability of a distance >= d under the null hypothesis (M3)."""
+def ks_probability(d, na, nb):
+    """Q_KS: probability of a distance >= d under the null hypothesis (M3).  The alternating series is summed
+    until its terms vanish in fp64 (about 3/lambda terms); below lambda = 0.04 Q_KS = 1 to 1e-300."""
     ne = float(na) * float(nb) / (float(na) + float(nb))
     lam = (np.sqrt(ne) + 0.12 + 0.11 / np.sqrt(ne)) * float(d)
-    if lam < 1e-3:
-        return 1.0                          # the alternating series does not converge at lambda -> 0; Q -> 1
-    total = 0.0
-    for j in range(1, terms + 1):
-        total += (-1.0) ** (j - 1) * np.exp(-2.0 * j * j * lam * lam)
+    if lam < 0.04:
+        return 1.0
+    total, j = 0.0, 1
+    while True:
+        term = np.exp(-2.0 * j * j * lam * lam)
+        total += term if j % 2 else -term
+        if term < 1e-20:
+            break
+        j += 1
     return float(min(1.0, max(0.0, 2.0 * total)))
 
 

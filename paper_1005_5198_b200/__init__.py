@@ -10,6 +10,8 @@ from .binding import (  # noqa: F401
     ML_ERR_INVALID_ARG,
     ML_ERR_OOM,
     ML_ERR_STATE,
+    ML_MEM_DEVICE,
+    ML_MEM_HOST,
     ML_OK,
     ML_PREC_FP32_COMPENSATED,
     ML_PREC_FP32_TILED,
@@ -20,11 +22,13 @@ from .binding import (  # noqa: F401
     ml_attach_stream,
     ml_capture_region,
     ml_create,
+    ml_delta_m_histogram,
     ml_destroy,
     ml_get_info,
     ml_get_map,
     ml_get_map_device,
     ml_get_stats,
+    ml_map_compare,
     ml_probe,
     ml_set_lenses,
     ml_set_precision,

@@ -28,7 +28,11 @@ EXPORTS = (
     "ml_create", "ml_destroy", "ml_get_info", "ml_set_lenses", "ml_set_precision", "ml_shoot",
     "ml_shoot_region", "ml_get_map", "ml_get_map_device", "ml_use_device_map", "ml_attach_stream",
     "ml_get_stats", "ml_capture_region", "ml_probe", "ml_strerror", "ml_version",
+    "ml_map_compare", "ml_delta_m_histogram",
 )
+
+ML_MEM_HOST = 0
+ML_MEM_DEVICE = 1
 
 
 class MlInfo(C.Structure):
@@ -47,6 +51,15 @@ class MlStats(C.Structure):
         ("rays_shot", C.c_uint64), ("rays_in_map", C.c_uint64), ("rays_dropped", C.c_uint64),
         ("interactions", C.c_uint64), ("kernel_launches", C.c_uint64),
         ("kernel_ms", C.c_double), ("total_ms", C.c_double),
+    ]
+
+
+class MlMapCompareResult(C.Structure):
+    _fields_ = [
+        ("n_pixels", C.c_uint64), ("n_valid", C.c_uint64), ("n_empty_a", C.c_uint64), ("n_empty_b", C.c_uint64),
+        ("sum_a", C.c_uint64), ("sum_b", C.c_uint64), ("max_a", C.c_uint32), ("max_b", C.c_uint32),
+        ("mean_mu_a", C.c_double), ("mean_mu_b", C.c_double), ("rms_delta_m", C.c_double),
+        ("ks_d", C.c_double), ("ks_prob", C.c_double), ("kernel_ms", C.c_double),
     ]
 
 
@@ -93,6 +106,10 @@ def load():
     lib.ml_get_stats.argtypes = [vp, C.POINTER(MlStats)]
     lib.ml_capture_region.argtypes = [vp, i64, i64, i64, i64, C.POINTER(dbl)]
     lib.ml_probe.argtypes = [vp, i64, C.POINTER(i64), C.POINTER(i64), C.POINTER(dbl)]
+    u32p = C.POINTER(C.c_uint32)
+    lib.ml_map_compare.argtypes = [vp, dbl, vp, dbl, i64, C.c_int, i32, vp, C.POINTER(MlMapCompareResult)]
+    lib.ml_delta_m_histogram.argtypes = [vp, dbl, i64, dbl, dbl, i32, C.c_int, i32, vp, C.POINTER(C.c_uint64)]
+    del u32p
     lib.ml_strerror.argtypes = [C.c_int]
     lib.ml_strerror.restype = C.c_char_p
     lib.ml_version.argtypes = []
@@ -204,4 +221,37 @@ def ml_probe(ctx, ray_i, ray_j) -> np.ndarray:
     ip = C.POINTER(C.c_int64)
     _check(load().ml_probe(ctx, ri.size, ri.ctypes.data_as(ip), rj.ctypes.data_as(ip),
                            out.ctypes.data_as(C.POINTER(C.c_double))), "ml_probe")
+    return out
+
+
+def _map_arg(m, n=None):
+    """(pointer, n, where, keepalive): a host uint32 array, or an int DEVICE pointer with n given."""
+    if isinstance(m, (int, np.integer)):
+        if n is None:
+            raise ValueError("a device pointer needs n")
+        return C.c_void_p(int(m)), int(n), ML_MEM_DEVICE, None
+    a = np.ascontiguousarray(m, dtype=np.uint32)
+    return C.c_void_p(a.ctypes.data), a.size, ML_MEM_HOST, a
+
+
+def ml_map_compare(a, n_rays_a, b, n_rays_b, n=None, device=0, cuda_stream=None) -> dict:
+    """RMS difference in magnitudes and two-sample K-S test between two count maps.
+    a, b: host uint32 arrays, or int device pointers (then pass n)."""
+    pa, na_, wa, ka = _map_arg(a, n)
+    pb, nb_, wb, kb = _map_arg(b, n)
+    if wa != wb or na_ != nb_:
+        raise ValueError("ml_map_compare: both maps must live in the same memory space and have the same size")
+    r = MlMapCompareResult()
+    _check(load().ml_map_compare(pa, float(n_rays_a), pb, float(n_rays_b), na_, wa, int(device),
+                                 C.c_void_p(int(cuda_stream) if cuda_stream else None), C.byref(r)), "ml_map_compare")
+    return _struct_dict(r)
+
+
+def ml_delta_m_histogram(counts, n_rays, lo, hi, n_bins, n=None, device=0, cuda_stream=None) -> np.ndarray:
+    """Histogram (uint64[n_bins]) of Delta m = -2.5 log10(count / n_rays) over [lo, hi) (eq. 10)."""
+    pc, n_, w, keep = _map_arg(counts, n)
+    out = np.zeros(int(n_bins), dtype=np.uint64)
+    _check(load().ml_delta_m_histogram(pc, float(n_rays), n_, float(lo), float(hi), int(n_bins), w, int(device),
+                                       C.c_void_p(int(cuda_stream) if cuda_stream else None),
+                                       out.ctypes.data_as(C.POINTER(C.c_uint64))), "ml_delta_m_histogram")
     return out

@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libmicrolens_b200.so")
-SOURCES = [os.path.join(CSRC, "microlens.cu")]
+SOURCES = [os.path.join(CSRC, "microlens.cu"), os.path.join(CSRC, "mapstats.cu")]
 DEPENDS = SOURCES + [os.path.join(CSRC, "shoot_kernel.cuh"), os.path.join(_ROOT, "include", "microlens.h")]
 
 NVCC_FLAGS = [

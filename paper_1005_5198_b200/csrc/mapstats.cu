@@ -1,0 +1,462 @@
+// mapstats.cu -- map comparison on the device (include/microlens.h, "Map comparison").
+//
+// The paper's two accuracy measures between magnification maps (section 3.1):
+// RMS difference in magnitudes and a two-sample Kolmogorov-Smirnov test on the distributions of
+// Delta m = -2.5 log10(mu) (eq. 10), mu = N/N_rays (eq. 3).
+//
+// Counts are integers, so the K-S distance needs no sort: one fused pass over both maps gathers
+// the RMS sums, the map statistics and the two count histograms (warp-aggregated RED into L2);
+// prefix sums of the histograms are the two empirical distributions, and
+//   D = max over sample points x of |F_a(x) - F_b(x)|
+// is evaluated at the sample points of both maps (x = c/n_rays_a and x = c/n_rays_b, compared in
+// mu, which orders the samples exactly as Delta m does, reversed).  All sums that feed a
+// floating-point result are reduced in a fixed order: results are bit-reproducible.
+#include "../../include/microlens.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+namespace mlstats {
+
+constexpr int kThreads = 256;
+constexpr unsigned int kCap0 = 1u << 20;  // bins of the first-pass count histograms
+constexpr unsigned int kCapMax = 1u << 27;
+constexpr int kScanItems = 16;            // elements per thread in the scan kernels
+constexpr int kScanTile = kThreads * kScanItems;
+
+struct Partial {
+    double ssq;                       // sum of (dm_a - dm_b)^2 over valid pixels
+    unsigned long long n_valid, n_empty_a, n_empty_b, sum_a, sum_b;
+    unsigned int max_a, max_b;
+};
+
+__device__ __forceinline__ void hist_add(unsigned int *hist, unsigned int cap, unsigned int c, bool active)
+{
+    // warp-aggregated: lanes holding the same count elect one leader that adds their number
+    const unsigned int mask = __ballot_sync(0xffffffffu, active);
+    if (!active) return;
+    const unsigned int peers = __match_any_sync(mask, c);
+    if ((__ffs(peers) - 1) == (int)(threadIdx.x & 31) && c < cap) atomicAdd(&hist[c], (unsigned int)__popc(peers));
+}
+
+// One pass over the maps: RMS sums, statistics, count histograms.  STATS = false: histograms only
+// (second pass when a count exceeded the first-pass bins).
+template <bool TWO, bool STATS>
+__global__ void __launch_bounds__(kThreads) pass_kernel(const unsigned int *__restrict__ a, const unsigned int *__restrict__ b,
+                                                        long long n, double n_rays_a, double n_rays_b, unsigned int *hist_a,
+                                                        unsigned int *hist_b, unsigned int cap, Partial *partials)
+{
+    Partial p;
+    p.ssq = 0.0;
+    p.n_valid = p.n_empty_a = p.n_empty_b = p.sum_a = p.sum_b = 0ull;
+    p.max_a = p.max_b = 0u;
+    const bool vec = ((reinterpret_cast<uintptr_t>(a) & 15) == 0) && (!TWO || (reinterpret_cast<uintptr_t>(b) & 15) == 0);
+    const long long stride = (long long)gridDim.x * kThreads * 4;
+    // every lane of a warp runs the same number of iterations (hist_add uses warp votes)
+    const long long warp_base = ((long long)blockIdx.x * kThreads + (threadIdx.x & ~31)) * 4;
+    for (long long w0 = warp_base; w0 < n; w0 += stride) {
+        const long long i = w0 + (threadIdx.x & 31) * 4;
+        unsigned int ca[4] = {0, 0, 0, 0}, cb[4] = {0, 0, 0, 0};
+        if (vec && i + 3 < n) {
+            const uint4 va = *reinterpret_cast<const uint4 *>(a + i);
+            ca[0] = va.x; ca[1] = va.y; ca[2] = va.z; ca[3] = va.w;
+            if (TWO) {
+                const uint4 vb = *reinterpret_cast<const uint4 *>(b + i);
+                cb[0] = vb.x; cb[1] = vb.y; cb[2] = vb.z; cb[3] = vb.w;
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (i + q < n) {
+                    ca[q] = a[i + q];
+                    if (TWO) cb[q] = b[i + q];
+                }
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const bool in = i + q < n;
+            hist_add(hist_a, cap, ca[q], in);
+            if (TWO) hist_add(hist_b, cap, cb[q], in);
+            if (STATS && in) {
+                p.sum_a += ca[q];
+                p.max_a = max(p.max_a, ca[q]);
+                p.n_empty_a += (ca[q] == 0);
+                if (TWO) {
+                    p.sum_b += cb[q];
+                    p.max_b = max(p.max_b, cb[q]);
+                    p.n_empty_b += (cb[q] == 0);
+                    if (ca[q] > 0 && cb[q] > 0) {
+                        // dm_a - dm_b = -2.5 log10( (N_a/n_rays_a) / (N_b/n_rays_b) )   (eq. 10)
+                        const double d = -2.5 * log10(((double)ca[q] / n_rays_a) / ((double)cb[q] / n_rays_b));
+                        p.ssq += d * d;
+                        p.n_valid += 1;
+                    }
+                }
+            }
+        }
+    }
+    if constexpr (STATS) {
+    // block reduction in a fixed order: lanes by shuffle tree, then warps in index order
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        p.ssq += __shfl_down_sync(0xffffffffu, p.ssq, o);
+        p.n_valid += __shfl_down_sync(0xffffffffu, p.n_valid, o);
+        p.n_empty_a += __shfl_down_sync(0xffffffffu, p.n_empty_a, o);
+        p.n_empty_b += __shfl_down_sync(0xffffffffu, p.n_empty_b, o);
+        p.sum_a += __shfl_down_sync(0xffffffffu, p.sum_a, o);
+        p.sum_b += __shfl_down_sync(0xffffffffu, p.sum_b, o);
+        p.max_a = max(p.max_a, __shfl_down_sync(0xffffffffu, p.max_a, o));
+        p.max_b = max(p.max_b, __shfl_down_sync(0xffffffffu, p.max_b, o));
+    }
+    __shared__ Partial wp[kThreads / 32];
+    if ((threadIdx.x & 31) == 0) wp[threadIdx.x >> 5] = p;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        Partial t = wp[0];
+        for (int w = 1; w < kThreads / 32; ++w) {
+            t.ssq += wp[w].ssq;
+            t.n_valid += wp[w].n_valid; t.n_empty_a += wp[w].n_empty_a; t.n_empty_b += wp[w].n_empty_b;
+            t.sum_a += wp[w].sum_a; t.sum_b += wp[w].sum_b;
+            t.max_a = max(t.max_a, wp[w].max_a); t.max_b = max(t.max_b, wp[w].max_b);
+        }
+        partials[blockIdx.x] = t;
+    }
+    } // STATS
+}
+
+// Sum the per-block partials in block order (one thread: a few thousand additions).
+__global__ void reduce_partials_kernel(const Partial *partials, int n_blocks, Partial *out)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    Partial t = partials[0];
+    for (int k = 1; k < n_blocks; ++k) {
+        const Partial q = partials[k];
+        t.ssq += q.ssq;
+        t.n_valid += q.n_valid; t.n_empty_a += q.n_empty_a; t.n_empty_b += q.n_empty_b;
+        t.sum_a += q.sum_a; t.sum_b += q.sum_b;
+        t.max_a = max(t.max_a, q.max_a); t.max_b = max(t.max_b, q.max_b);
+    }
+    *out = t;
+}
+
+// ---- inclusive prefix sums of a count histogram (three small kernels, tiles of kScanTile bins)
+__global__ void __launch_bounds__(kThreads) scan_tile_sums_kernel(const unsigned int *hist, unsigned int cap, unsigned int *tile_sums)
+{
+    const unsigned int base = blockIdx.x * kScanTile;
+    unsigned int s = 0;
+    for (int q = 0; q < kScanItems; ++q) {
+        const unsigned int k = base + q * kThreads + threadIdx.x;
+        if (k < cap) s += hist[k];
+    }
+    __shared__ unsigned int ws[kThreads / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned int t = 0;
+        for (int w = 0; w < kThreads / 32; ++w) t += ws[w];
+        tile_sums[blockIdx.x] = t;
+    }
+}
+
+__global__ void scan_tile_offsets_kernel(unsigned int *tile_sums, int n_tiles)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    unsigned int run = 0;
+    for (int k = 0; k < n_tiles; ++k) {
+        const unsigned int v = tile_sums[k];
+        tile_sums[k] = run; // exclusive
+        run += v;
+    }
+}
+
+__global__ void __launch_bounds__(kThreads) scan_apply_kernel(const unsigned int *hist, unsigned int cap, const unsigned int *tile_offsets,
+                                                              unsigned int *cum)
+{
+    // thread t owns the kScanItems consecutive bins starting at base + t*kScanItems
+    const unsigned int base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
+    unsigned int v[kScanItems];
+    unsigned int s = 0;
+#pragma unroll
+    for (int q = 0; q < kScanItems; ++q) {
+        v[q] = (base + q < cap) ? hist[base + q] : 0u;
+        s += v[q];
+    }
+    // exclusive scan of the per-thread sums over the block
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    unsigned int incl = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int u = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += u;
+    }
+    __shared__ unsigned int ws[kThreads / 32];
+    if (lane == 31) ws[warp] = incl;
+    __syncthreads();
+    unsigned int off = tile_offsets[blockIdx.x];
+    for (int w = 0; w < warp; ++w) off += ws[w];
+    unsigned int run = off + incl - s;
+#pragma unroll
+    for (int q = 0; q < kScanItems; ++q) {
+        run += v[q];
+        if (base + q < cap) cum[base + q] = run;
+    }
+}
+
+// floor(c * num / den) clipped to `last`; exact when num, den have <= 26 significant bits.
+__device__ __forceinline__ unsigned int floor_ratio(unsigned int c, double num, double den, unsigned int last)
+{
+    const double t = (double)c * num;
+    double q = floor(t / den);
+    if ((q + 1.0) * den <= t) q += 1.0;
+    else if (q * den > t) q -= 1.0;
+    if (q >= (double)last) return last;
+    return q < 0.0 ? 0u : (unsigned int)q;
+}
+
+// D = max_x |F_a(x) - F_b(x)| at the sample points of both maps (x in mu = count / n_rays).
+__global__ void __launch_bounds__(kThreads) ks_kernel(const unsigned int *cum_a, const unsigned int *cum_b, unsigned int cap, double n,
+                                                      double n_rays_a, double n_rays_b, unsigned long long *d_bits)
+{
+    double d = 0.0;
+    const unsigned int last = cap - 1;
+    for (unsigned int c = blockIdx.x * kThreads + threadIdx.x; c < cap; c += gridDim.x * kThreads) {
+        // x = c / n_rays_a : F_a = cum_a[c], F_b = #{N_b <= c n_rays_b / n_rays_a}
+        const double fa1 = (double)cum_a[c] / n, fb1 = (double)cum_b[floor_ratio(c, n_rays_b, n_rays_a, last)] / n;
+        // x = c / n_rays_b
+        const double fb2 = (double)cum_b[c] / n, fa2 = (double)cum_a[floor_ratio(c, n_rays_a, n_rays_b, last)] / n;
+        d = fmax(d, fmax(fabs(fa1 - fb1), fabs(fa2 - fb2)));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) d = fmax(d, __shfl_down_sync(0xffffffffu, d, o));
+    if ((threadIdx.x & 31) == 0 && d > 0.0) atomicMax(d_bits, (unsigned long long)__double_as_longlong(d)); // d >= 0: bit order = value order
+}
+
+// Delta m histogram from the count histogram: one evaluation of eq. 10 per distinct count.
+__global__ void __launch_bounds__(kThreads) delta_m_hist_kernel(const unsigned int *hist, unsigned int cap, double n_rays, double lo, double hi,
+                                                                int n_bins, unsigned long long *out)
+{
+    const double w = (hi - lo) / (double)n_bins;
+    for (unsigned int c = 1 + blockIdx.x * kThreads + threadIdx.x; c < cap; c += gridDim.x * kThreads) {
+        const unsigned int h = hist[c];
+        if (!h) continue;
+        const double x = -2.5 * log10((double)c / n_rays);
+        if (!(x >= lo)) continue;
+        const double k = floor((x - lo) / w);
+        if (k >= 0.0 && k < (double)n_bins) atomicAdd(&out[(int)k], (unsigned long long)h);
+    }
+}
+
+// Q_KS(lambda) = 2 sum_{j>=1} (-1)^(j-1) exp(-2 j^2 lambda^2), lambda = (sqrt(Ne) + 0.12 + 0.11/sqrt(Ne)) D.
+__global__ void finalize_kernel(const Partial *tot, const unsigned long long *d_bits, double n, double n_rays_a, double n_rays_b,
+                                ml_map_compare_result *out)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const Partial t = *tot;
+    ml_map_compare_result r;
+    r.n_pixels = (uint64_t)n;
+    r.n_valid = t.n_valid; r.n_empty_a = t.n_empty_a; r.n_empty_b = t.n_empty_b;
+    r.sum_a = t.sum_a; r.sum_b = t.sum_b; r.max_a = t.max_a; r.max_b = t.max_b;
+    r.mean_mu_a = ((double)t.sum_a / n) / n_rays_a;
+    r.mean_mu_b = ((double)t.sum_b / n) / n_rays_b;
+    r.rms_delta_m = t.n_valid ? sqrt(t.ssq / (double)t.n_valid) : 0.0;
+    const double d = __longlong_as_double((long long)*d_bits);
+    r.ks_d = d;
+    const double ne = n * n / (n + n);
+    const double lam = (sqrt(ne) + 0.12 + 0.11 / sqrt(ne)) * d;
+    // two series for the same function: the theta-function form converges fast where the alternating one does not
+    double q;
+    if (lam < 0.04) {
+        q = 1.0;
+    } else if (lam < 1.18) {
+        const double y = exp(-1.2337005501361697 / (lam * lam)); // exp(-pi^2 / (8 lambda^2))
+        const double y2 = y * y, y4 = y2 * y2, y8 = y4 * y4;
+        // sum_{j=1..4} y^((2j-1)^2) = y + y^9 + y^25 + y^49
+        q = 1.0 - (2.5066282746310002 / lam) * (y + y8 * y + y8 * y8 * y8 * y + y8 * y8 * y8 * y8 * y8 * y8 * y);
+    } else {
+        const double x = exp(-2.0 * lam * lam);
+        const double x2 = x * x, x4 = x2 * x2, x8 = x4 * x4;
+        // sum_{j=1..4} (-1)^(j-1) x^(j^2) = x - x^4 + x^9 - x^16
+        q = 2.0 * (x - x4 + x8 * x - x8 * x8);
+    }
+    q = fmin(1.0, fmax(0.0, q));
+    r.ks_prob = q;
+    r.kernel_ms = 0.0;
+    *out = r;
+}
+
+} // namespace mlstats
+
+// ---------------------------------------------------------------------------------------- host side
+namespace {
+
+using namespace mlstats;
+
+struct StatsGuard { // device selection + everything the call allocates
+    int prev = 0;
+    bool ok = false;
+    void *ptrs[20];
+    int n_ptrs = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    explicit StatsGuard(int dev)
+    {
+        int ndev = 0;
+        if (cudaGetDeviceCount(&ndev) != cudaSuccess || dev < 0 || dev >= ndev) { cudaGetLastError(); return; }
+        if (cudaGetDevice(&prev) != cudaSuccess) return;
+        ok = (prev == dev) || (cudaSetDevice(dev) == cudaSuccess);
+    }
+    template <typename T> T *alloc(size_t count)
+    {
+        void *p = nullptr;
+        if (n_ptrs >= 20 || cudaMalloc(&p, (count ? count : 1) * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        ptrs[n_ptrs++] = p;
+        return static_cast<T *>(p);
+    }
+    ~StatsGuard()
+    {
+        for (int k = 0; k < n_ptrs; ++k) cudaFree(ptrs[k]);
+        if (ev0) cudaEventDestroy(ev0);
+        if (ev1) cudaEventDestroy(ev1);
+        if (ok) cudaSetDevice(prev);
+    }
+};
+
+int grid_for(long long n, int sm_count)
+{
+    const long long want = (n + (long long)kThreads * 4 - 1) / ((long long)kThreads * 4);
+    const long long cap = (long long)sm_count * 8; // 8 resident CTAs of 256 threads per SM
+    return (int)(want < 1 ? 1 : (want < cap ? want : cap));
+}
+
+// inclusive prefix sums of hist[0..cap) into cum[0..cap)
+bool scan_hist(const unsigned int *hist, unsigned int cap, unsigned int *tile_sums, unsigned int *cum, cudaStream_t s)
+{
+    const int n_tiles = (int)((cap + kScanTile - 1) / kScanTile);
+    scan_tile_sums_kernel<<<n_tiles, kThreads, 0, s>>>(hist, cap, tile_sums);
+    scan_tile_offsets_kernel<<<1, 32, 0, s>>>(tile_sums, n_tiles);
+    scan_apply_kernel<<<n_tiles, kThreads, 0, s>>>(hist, cap, tile_sums, cum);
+    return cudaGetLastError() == cudaSuccess;
+}
+
+// Shared front half of both entry points: device copies of the maps, the fused pass, the reduced
+// statistics on the host, and count histograms that hold every count (cap_eff bins used).
+struct PassOut {
+    const unsigned int *da = nullptr, *db = nullptr;
+    unsigned int *hist_a = nullptr, *hist_b = nullptr;
+    Partial *d_total = nullptr;
+    Partial total;
+    unsigned int cap_eff = 0;
+    int sm_count = 0;
+};
+
+int run_pass(StatsGuard &g, cudaStream_t s, const uint32_t *a, const uint32_t *b, int64_t n, double na, double nb, int where,
+             int device, PassOut &o)
+{
+    if (cudaDeviceGetAttribute(&o.sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return ML_ERR_CUDA;
+    const bool two = b != nullptr;
+    o.da = a; o.db = b;
+    if (where == ML_MEM_HOST) {
+        unsigned int *ta = g.alloc<unsigned int>((size_t)n), *tb = two ? g.alloc<unsigned int>((size_t)n) : nullptr;
+        if (!ta || (two && !tb)) return ML_ERR_OOM;
+        if (cudaMemcpyAsync(ta, a, (size_t)n * 4, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+            (two && cudaMemcpyAsync(tb, b, (size_t)n * 4, cudaMemcpyHostToDevice, s) != cudaSuccess))
+            return ML_ERR_CUDA;
+        o.da = ta; o.db = tb;
+    }
+    const int grid = grid_for(n, o.sm_count);
+    Partial *partials = g.alloc<Partial>((size_t)grid);
+    o.d_total = g.alloc<Partial>(1);
+    o.hist_a = g.alloc<unsigned int>(kCap0);
+    o.hist_b = two ? g.alloc<unsigned int>(kCap0) : nullptr;
+    if (!partials || !o.d_total || !o.hist_a || (two && !o.hist_b)) return ML_ERR_OOM;
+    if (cudaEventCreate(&g.ev0) != cudaSuccess || cudaEventCreate(&g.ev1) != cudaSuccess) return ML_ERR_CUDA;
+    if (cudaEventRecord(g.ev0, s) != cudaSuccess) return ML_ERR_CUDA;
+    if (cudaMemsetAsync(o.hist_a, 0, kCap0 * 4ull, s) != cudaSuccess || (two && cudaMemsetAsync(o.hist_b, 0, kCap0 * 4ull, s) != cudaSuccess))
+        return ML_ERR_CUDA;
+    if (two) pass_kernel<true, true><<<grid, kThreads, 0, s>>>(o.da, o.db, n, na, nb, o.hist_a, o.hist_b, kCap0, partials);
+    else pass_kernel<false, true><<<grid, kThreads, 0, s>>>(o.da, nullptr, n, na, nb, o.hist_a, nullptr, kCap0, partials);
+    reduce_partials_kernel<<<1, 32, 0, s>>>(partials, grid, o.d_total);
+    if (cudaGetLastError() != cudaSuccess) return ML_ERR_CUDA;
+    if (cudaMemcpyAsync(&o.total, o.d_total, sizeof(Partial), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+        return ML_ERR_CUDA;
+    const unsigned int mx = o.total.max_a > o.total.max_b ? o.total.max_a : o.total.max_b;
+    if (mx >= kCapMax) return ML_ERR_OOM;
+    o.cap_eff = mx + 1;
+    if (o.cap_eff > kCap0) { // a count beyond the first-pass bins: histogram again with enough of them
+        o.hist_a = g.alloc<unsigned int>(o.cap_eff);
+        o.hist_b = two ? g.alloc<unsigned int>(o.cap_eff) : nullptr;
+        if (!o.hist_a || (two && !o.hist_b)) return ML_ERR_OOM;
+        if (cudaMemsetAsync(o.hist_a, 0, (size_t)o.cap_eff * 4, s) != cudaSuccess ||
+            (two && cudaMemsetAsync(o.hist_b, 0, (size_t)o.cap_eff * 4, s) != cudaSuccess))
+            return ML_ERR_CUDA;
+        if (two) pass_kernel<true, false><<<grid, kThreads, 0, s>>>(o.da, o.db, n, na, nb, o.hist_a, o.hist_b, o.cap_eff, nullptr);
+        else pass_kernel<false, false><<<grid, kThreads, 0, s>>>(o.da, nullptr, n, na, nb, o.hist_a, nullptr, o.cap_eff, nullptr);
+        if (cudaGetLastError() != cudaSuccess) return ML_ERR_CUDA;
+    }
+    return ML_OK;
+}
+
+bool bad_rays(double v) { return !(v > 0.0) || !isfinite(v); }
+
+} // namespace
+
+extern "C" {
+
+int ml_map_compare(const uint32_t *a, double n_rays_a, const uint32_t *b, double n_rays_b, int64_t n, int where, int32_t device,
+                   void *cuda_stream, ml_map_compare_result *out)
+{
+    if (!a || !b || !out || n < 1 || n > 0x7fffffffLL || bad_rays(n_rays_a) || bad_rays(n_rays_b) ||
+        (where != ML_MEM_HOST && where != ML_MEM_DEVICE))
+        return ML_ERR_INVALID_ARG;
+    StatsGuard g(device);
+    if (!g.ok) return ML_ERR_CUDA;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    PassOut o;
+    int rc = run_pass(g, s, a, b, n, n_rays_a, n_rays_b, where, device, o);
+    if (rc != ML_OK) return rc;
+    const int n_tiles = (int)((o.cap_eff + kScanTile - 1) / kScanTile);
+    unsigned int *cum_a = g.alloc<unsigned int>(o.cap_eff), *cum_b = g.alloc<unsigned int>(o.cap_eff);
+    unsigned int *tiles = g.alloc<unsigned int>((size_t)n_tiles);
+    unsigned long long *d_bits = g.alloc<unsigned long long>(1);
+    ml_map_compare_result *d_res = g.alloc<ml_map_compare_result>(1);
+    if (!cum_a || !cum_b || !tiles || !d_bits || !d_res) return ML_ERR_OOM;
+    if (cudaMemsetAsync(d_bits, 0, 8, s) != cudaSuccess) return ML_ERR_CUDA;
+    if (!scan_hist(o.hist_a, o.cap_eff, tiles, cum_a, s) || !scan_hist(o.hist_b, o.cap_eff, tiles, cum_b, s)) return ML_ERR_CUDA;
+    const int ks_grid = (int)((o.cap_eff + kThreads - 1) / kThreads) < o.sm_count * 8 ? (int)((o.cap_eff + kThreads - 1) / kThreads) : o.sm_count * 8;
+    ks_kernel<<<ks_grid, kThreads, 0, s>>>(cum_a, cum_b, o.cap_eff, (double)n, n_rays_a, n_rays_b, d_bits);
+    finalize_kernel<<<1, 32, 0, s>>>(o.d_total, d_bits, (double)n, n_rays_a, n_rays_b, d_res);
+    if (cudaGetLastError() != cudaSuccess || cudaEventRecord(g.ev1, s) != cudaSuccess) return ML_ERR_CUDA;
+    if (cudaMemcpyAsync(out, d_res, sizeof(*out), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+        return ML_ERR_CUDA;
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, g.ev0, g.ev1) != cudaSuccess) return ML_ERR_CUDA;
+    out->kernel_ms = ms;
+    return ML_OK;
+}
+
+int ml_delta_m_histogram(const uint32_t *counts, double n_rays, int64_t n, double lo, double hi, int32_t n_bins, int where,
+                         int32_t device, void *cuda_stream, uint64_t *hist_out)
+{
+    if (!counts || !hist_out || n < 1 || n > 0x7fffffffLL || bad_rays(n_rays) || !(lo < hi) || !isfinite(lo) || !isfinite(hi) ||
+        n_bins < 1 || n_bins > (1 << 20) || (where != ML_MEM_HOST && where != ML_MEM_DEVICE))
+        return ML_ERR_INVALID_ARG;
+    StatsGuard g(device);
+    if (!g.ok) return ML_ERR_CUDA;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    PassOut o;
+    int rc = run_pass(g, s, counts, nullptr, n, n_rays, n_rays, where, device, o);
+    if (rc != ML_OK) return rc;
+    unsigned long long *d_out = g.alloc<unsigned long long>((size_t)n_bins);
+    if (!d_out) return ML_ERR_OOM;
+    if (cudaMemsetAsync(d_out, 0, (size_t)n_bins * 8, s) != cudaSuccess) return ML_ERR_CUDA;
+    const int want = (int)((o.cap_eff + kThreads - 1) / kThreads);
+    delta_m_hist_kernel<<<want < o.sm_count * 8 ? want : o.sm_count * 8, kThreads, 0, s>>>(o.hist_a, o.cap_eff, n_rays, lo, hi, n_bins, d_out);
+    if (cudaGetLastError() != cudaSuccess) return ML_ERR_CUDA;
+    if (cudaMemcpyAsync(hist_out, d_out, (size_t)n_bins * 8, cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
+        return ML_ERR_CUDA;
+    return ML_OK;
+}
+
+} // extern "C"

@@ -72,7 +72,8 @@ def test_ks_statistic_hand_worked_and_extremes():
 
 
 def test_ks_probability_is_the_kolmogorov_series_with_stephens_correction():
-    for d, na, nb in [(0.01, 4096, 4096), (0.02, 16384, 8000), (0.3, 20, 30), (0.001, 10 ** 6, 10 ** 6)]:
+    for d, na, nb in [(0.01, 4096, 4096), (0.02, 16384, 8000), (0.3, 20, 30), (0.001, 10 ** 6, 10 ** 6),
+                      (2e-4, 16384, 16384), (0.004, 16384, 16384), (0.0008, 16384, 16384), (0.03, 300, 200)]:
         ne = na * nb / (na + nb)
         lam = (math.sqrt(ne) + 0.12 + 0.11 / math.sqrt(ne)) * d
         assert abs(mo.ks_probability(d, na, nb) - special.kolmogorov(lam)) < 1e-12

@@ -314,6 +314,97 @@ def run_ours(args):
     return 0
 
 
+# ------------------------------------------------------------------ the map-comparison row
+def run_mapstats(args):
+    """--row mapstats: pixels/s of ml_map_compare (RMS in magnitudes + two-sample K-S) on two
+    seeded synthetic 4096^2 count maps (the map size of C4) resident in HBM; HBM roofline."""
+    import torch
+    import paper_1005_5198_b200 as ml
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    n_pix, n_rays = 4096, 100.0
+    rng = np.random.default_rng(5)
+    a = rng.poisson(5.0 * n_rays * rng.lognormal(0.0, 0.7, size=(n_pix, n_pix))).astype(np.uint32)
+    b = np.clip(a.astype(np.int64) + rng.integers(-30, 31, size=a.shape), 0, None).astype(np.uint32)
+    n = a.size
+    ta = torch.from_numpy(a.view(np.int32)).to(dev)
+    tb = torch.from_numpy(b.view(np.int32)).to(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.Stream(device=dev)
+
+    def step():
+        with torch.cuda.stream(stream):
+            flush.fill_(1)
+        return ml.ml_map_compare(ta.data_ptr(), n_rays, tb.data_ptr(), n_rays, n=n, device=dev.index,
+                                 cuda_stream=stream.cuda_stream)
+
+    sampler = ClockSampler(dev.index)
+    sampler.start()   # the timed region lasts a few ms: sample from the warm-up on so that some samples exist
+    for _ in range(args.warmup):
+        r = step()
+    torch.cuda.synchronize(dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kernel_ms, pass_ms = 0.0, 0.0
+    e0.record(stream)
+    for _ in range(args.steps):
+        r = step()
+        kernel_ms += r["kernel_ms"]
+        pass_ms += r["pass_kernel_ms"]
+    e1.record(stream)
+    torch.cuda.synchronize(dev)
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        r_host = ml.ml_map_compare(a, n_rays, b, n_rays, device=dev.index)   # host buffers: H2D inside
+    e2e_s = time.perf_counter() - t0
+    assert r_host["rms_delta_m"] == r["rms_delta_m"] and r_host["ks_d"] == r["ks_d"]
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    peak = float(peaks.get("hbm_gbs") or 6500.0)
+    algo_bytes = 2 * 4 * n
+    achieved = algo_bytes / (pass_ms / args.steps * 1e-3) / 1e9
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import mapstats_oracle as mo
+        sa, sb = a[:2048, :2048], b[:2048, :2048]
+        t0 = time.perf_counter()
+        rms, _ = mo.rms_delta_m(sa, n_rays, sb, n_rays)
+        d = mo.ks_statistic(sa, n_rays, sb, n_rays)
+        mo.ks_probability(d, sa.size, sb.size)
+        dt = time.perf_counter() - t0
+        cpu = {"value": sa.size / dt, "unit": "pixels/s", "cores": 1, "kind": "oracle",
+               "sample": "2048x2048 corner of the same two maps: rms + K-S distance + Q_KS in %.2f s" % dt}
+    line = {"metric": "map-comparison pixels/sec (RMS in magnitudes + two-sample K-S, PAPER.md:169-173)",
+            "value": n * args.steps / (ms * 1e-3), "unit": "pixels/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "mapstats: two seeded synthetic 4096^2 uint32 count maps (C4's map size), n_rays=100",
+                       "l2": "flushed between steps (256 MiB write); the two maps (134 MB) exceed L2 anyway"},
+            "result": {k: r[k] for k in ("rms_delta_m", "ks_d", "ks_prob", "n_valid")},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": 134337536 + 5088768, "pass_kernel_ms": pass_ms / args.steps,
+                         "all_kernels_ms_per_call": kernel_ms / args.steps,
+                         "note": "dominant kernel = mlstats::pass_kernel (fused RMS + statistics + count histograms); "
+                                 "algorithmic bytes = 2 maps x 4 B x n pixels read once; time = CUDA events around that "
+                                 "launch on the launching stream (ml_map_compare_result.pass_kernel_ms); traffic = ncu "
+                                 "dram bytes read + written of that launch (profiles/r01_ncu_full_mapstats.txt); "
+                                 "peak = MEASURED_PEAKS.json hbm_gbs"},
+            "cpu_baseline": cpu, "clocks": clocks,
+            "e2e": {"value": n * args.steps / e2e_s, "unit": "pixels/s", "h2d_bytes_per_step": 2 * 4 * n,
+                    "d2h_bytes_per_step": 112},
+            "gpu_launches": 11 * args.steps}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -322,11 +413,15 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C2", help="C1..C5 (BASELINE.json configs); the metric is quoted on C2")
     ap.add_argument("--precision", default="fp32_tiled", choices=sorted(PRECISIONS))
+    ap.add_argument("--row", default="shoot", choices=["shoot", "mapstats"],
+                    help="shoot = the hot path (default, the BASELINE.json metric); mapstats = the map-comparison row")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: note: --warmup < 3 breaks the timing rules", file=sys.stderr)
+    if args.row == "mapstats" and args.impl == "ours":
+        return run_mapstats(args)
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 
 

@@ -188,7 +188,9 @@ typedef struct {
                                       empty pixel is a sample at +inf, M2)                       */
     double ks_prob;                /* Q_KS((sqrt(Ne)+0.12+0.11/sqrt(Ne)) ks_d), Ne = n/2 (M3):
                                       probability of a distance >= ks_d under the null hypothesis */
-    double kernel_ms;              /* device time of the kernels, CUDA events on the stream      */
+    double kernel_ms;              /* device time of the whole call (all kernels, the memsets and
+                                      one small host read-back between them), CUDA events        */
+    double pass_kernel_ms;         /* device time of the fused pass over the maps alone          */
 } ml_map_compare_result;
 
 /* Compare two count maps of n pixels each (same layout; n >= 1).  a, b: uint32 counts in HOST or

@@ -59,7 +59,7 @@ class MlMapCompareResult(C.Structure):
         ("n_pixels", C.c_uint64), ("n_valid", C.c_uint64), ("n_empty_a", C.c_uint64), ("n_empty_b", C.c_uint64),
         ("sum_a", C.c_uint64), ("sum_b", C.c_uint64), ("max_a", C.c_uint32), ("max_b", C.c_uint32),
         ("mean_mu_a", C.c_double), ("mean_mu_b", C.c_double), ("rms_delta_m", C.c_double),
-        ("ks_d", C.c_double), ("ks_prob", C.c_double), ("kernel_ms", C.c_double),
+        ("ks_d", C.c_double), ("ks_prob", C.c_double), ("kernel_ms", C.c_double), ("pass_kernel_ms", C.c_double),
     ]
 
 

@@ -31,32 +31,46 @@ struct Partial {
     unsigned int max_a, max_b;
 };
 
-__device__ __forceinline__ void hist_add(unsigned int *hist, unsigned int cap, unsigned int c, bool active)
+constexpr int kPassThreads = 1024;        // one CTA per SM
+constexpr unsigned int kShBins = 16384;   // per map: counts below this are histogrammed in shared memory
+constexpr unsigned int kLut = 8192;       // log10(c) for c < kLut is tabulated per CTA in shared memory
+
+__device__ __forceinline__ void hist_add(unsigned int *sh, unsigned int *hist, unsigned int cap, unsigned int c)
 {
-    // warp-aggregated: lanes holding the same count elect one leader that adds their number
-    const unsigned int mask = __ballot_sync(0xffffffffu, active);
-    if (!active) return;
-    const unsigned int peers = __match_any_sync(mask, c);
-    if ((__ffs(peers) - 1) == (int)(threadIdx.x & 31) && c < cap) atomicAdd(&hist[c], (unsigned int)__popc(peers));
+    if (c < kShBins) {
+        atomicAdd(&sh[c], 1u);
+    } else if (c < cap) {
+        // rare, bright pixels: warp-aggregated RED into the global histogram
+        const unsigned int peers = __match_any_sync(__activemask(), c);
+        if ((__ffs(peers) - 1) == (int)(threadIdx.x & 31)) atomicAdd(&hist[c], (unsigned int)__popc(peers));
+    }
 }
 
-// One pass over the maps: RMS sums, statistics, count histograms.  STATS = false: histograms only
-// (second pass when a count exceeded the first-pass bins).
+// One pass over the maps: RMS sums, statistics, count histograms (privatised per CTA in shared memory for
+// counts < kShBins, flushed once at the end).  STATS = false: histograms only (second pass when a count
+// exceeded the first-pass bins).
 template <bool TWO, bool STATS>
-__global__ void __launch_bounds__(kThreads) pass_kernel(const unsigned int *__restrict__ a, const unsigned int *__restrict__ b,
-                                                        long long n, double n_rays_a, double n_rays_b, unsigned int *hist_a,
-                                                        unsigned int *hist_b, unsigned int cap, Partial *partials)
+__global__ void __launch_bounds__(kPassThreads, 1) pass_kernel(const unsigned int *__restrict__ a, const unsigned int *__restrict__ b,
+                                                               long long n, double n_rays_a, double n_rays_b, unsigned int *hist_a,
+                                                               unsigned int *hist_b, unsigned int cap, Partial *partials)
 {
+    extern __shared__ __align__(8) unsigned char sh_raw[]; // [kLut] doubles, then [kShBins] bins for a and for b
+    double *sh_log = reinterpret_cast<double *>(sh_raw);
+    unsigned int *sh_hist = reinterpret_cast<unsigned int *>(sh_raw + kLut * sizeof(double));
+    unsigned int *sh_a = sh_hist, *sh_b = sh_hist + kShBins;
+    for (unsigned int k = threadIdx.x; k < (TWO ? 2 : 1) * kShBins; k += kPassThreads) sh_hist[k] = 0u;
+    if (TWO && STATS)
+        for (unsigned int k = threadIdx.x; k < kLut; k += kPassThreads) sh_log[k] = log10((double)k); // [0] = -inf, never read
+    const double log_rays = (n_rays_a == n_rays_b) ? 0.0 : log10(n_rays_a / n_rays_b);
+    __syncthreads();
+
     Partial p;
     p.ssq = 0.0;
     p.n_valid = p.n_empty_a = p.n_empty_b = p.sum_a = p.sum_b = 0ull;
     p.max_a = p.max_b = 0u;
     const bool vec = ((reinterpret_cast<uintptr_t>(a) & 15) == 0) && (!TWO || (reinterpret_cast<uintptr_t>(b) & 15) == 0);
-    const long long stride = (long long)gridDim.x * kThreads * 4;
-    // every lane of a warp runs the same number of iterations (hist_add uses warp votes)
-    const long long warp_base = ((long long)blockIdx.x * kThreads + (threadIdx.x & ~31)) * 4;
-    for (long long w0 = warp_base; w0 < n; w0 += stride) {
-        const long long i = w0 + (threadIdx.x & 31) * 4;
+    const long long stride = (long long)gridDim.x * kPassThreads * 4;
+    for (long long i = ((long long)blockIdx.x * kPassThreads + threadIdx.x) * 4; i < n; i += stride) {
         unsigned int ca[4] = {0, 0, 0, 0}, cb[4] = {0, 0, 0, 0};
         if (vec && i + 3 < n) {
             const uint4 va = *reinterpret_cast<const uint4 *>(a + i);
@@ -75,10 +89,10 @@ __global__ void __launch_bounds__(kThreads) pass_kernel(const unsigned int *__re
         }
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            const bool in = i + q < n;
-            hist_add(hist_a, cap, ca[q], in);
-            if (TWO) hist_add(hist_b, cap, cb[q], in);
-            if (STATS && in) {
+            if (i + q >= n) break;
+            hist_add(sh_a, hist_a, cap, ca[q]);
+            if (TWO) hist_add(sh_b, hist_b, cap, cb[q]);
+            if (STATS) {
                 p.sum_a += ca[q];
                 p.max_a = max(p.max_a, ca[q]);
                 p.n_empty_a += (ca[q] == 0);
@@ -87,8 +101,10 @@ __global__ void __launch_bounds__(kThreads) pass_kernel(const unsigned int *__re
                     p.max_b = max(p.max_b, cb[q]);
                     p.n_empty_b += (cb[q] == 0);
                     if (ca[q] > 0 && cb[q] > 0) {
-                        // dm_a - dm_b = -2.5 log10( (N_a/n_rays_a) / (N_b/n_rays_b) )   (eq. 10)
-                        const double d = -2.5 * log10(((double)ca[q] / n_rays_a) / ((double)cb[q] / n_rays_b));
+                        // dm_a - dm_b = -2.5 (log10 N_a - log10 N_b - log10(n_rays_a / n_rays_b))   (eq. 10)
+                        const double la = ca[q] < kLut ? sh_log[ca[q]] : log10((double)ca[q]);
+                        const double lb = cb[q] < kLut ? sh_log[cb[q]] : log10((double)cb[q]);
+                        const double d = -2.5 * ((la - lb) - log_rays);
                         p.ssq += d * d;
                         p.n_valid += 1;
                     }
@@ -96,48 +112,75 @@ __global__ void __launch_bounds__(kThreads) pass_kernel(const unsigned int *__re
             }
         }
     }
-    if constexpr (STATS) {
-    // block reduction in a fixed order: lanes by shuffle tree, then warps in index order
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        p.ssq += __shfl_down_sync(0xffffffffu, p.ssq, o);
-        p.n_valid += __shfl_down_sync(0xffffffffu, p.n_valid, o);
-        p.n_empty_a += __shfl_down_sync(0xffffffffu, p.n_empty_a, o);
-        p.n_empty_b += __shfl_down_sync(0xffffffffu, p.n_empty_b, o);
-        p.sum_a += __shfl_down_sync(0xffffffffu, p.sum_a, o);
-        p.sum_b += __shfl_down_sync(0xffffffffu, p.sum_b, o);
-        p.max_a = max(p.max_a, __shfl_down_sync(0xffffffffu, p.max_a, o));
-        p.max_b = max(p.max_b, __shfl_down_sync(0xffffffffu, p.max_b, o));
-    }
-    __shared__ Partial wp[kThreads / 32];
-    if ((threadIdx.x & 31) == 0) wp[threadIdx.x >> 5] = p;
     __syncthreads();
-    if (threadIdx.x == 0) {
-        Partial t = wp[0];
-        for (int w = 1; w < kThreads / 32; ++w) {
-            t.ssq += wp[w].ssq;
-            t.n_valid += wp[w].n_valid; t.n_empty_a += wp[w].n_empty_a; t.n_empty_b += wp[w].n_empty_b;
-            t.sum_a += wp[w].sum_a; t.sum_b += wp[w].sum_b;
-            t.max_a = max(t.max_a, wp[w].max_a); t.max_b = max(t.max_b, wp[w].max_b);
+    for (unsigned int k = threadIdx.x; k < kShBins; k += kPassThreads) {
+        const unsigned int va = sh_a[k];
+        if (va) atomicAdd(&hist_a[k], va);
+        if (TWO) {
+            const unsigned int vb = sh_b[k];
+            if (vb) atomicAdd(&hist_b[k], vb);
         }
-        partials[blockIdx.x] = t;
     }
-    } // STATS
+    if constexpr (STATS) {
+        // block reduction in a fixed order: lanes by shuffle tree, then warps in index order
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            p.ssq += __shfl_down_sync(0xffffffffu, p.ssq, o);
+            p.n_valid += __shfl_down_sync(0xffffffffu, p.n_valid, o);
+            p.n_empty_a += __shfl_down_sync(0xffffffffu, p.n_empty_a, o);
+            p.n_empty_b += __shfl_down_sync(0xffffffffu, p.n_empty_b, o);
+            p.sum_a += __shfl_down_sync(0xffffffffu, p.sum_a, o);
+            p.sum_b += __shfl_down_sync(0xffffffffu, p.sum_b, o);
+            p.max_a = max(p.max_a, __shfl_down_sync(0xffffffffu, p.max_a, o));
+            p.max_b = max(p.max_b, __shfl_down_sync(0xffffffffu, p.max_b, o));
+        }
+        __shared__ Partial wp[kPassThreads / 32];
+        if ((threadIdx.x & 31) == 0) wp[threadIdx.x >> 5] = p;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            Partial t = wp[0];
+            for (int w = 1; w < kPassThreads / 32; ++w) {
+                t.ssq += wp[w].ssq;
+                t.n_valid += wp[w].n_valid; t.n_empty_a += wp[w].n_empty_a; t.n_empty_b += wp[w].n_empty_b;
+                t.sum_a += wp[w].sum_a; t.sum_b += wp[w].sum_b;
+                t.max_a = max(t.max_a, wp[w].max_a); t.max_b = max(t.max_b, wp[w].max_b);
+            }
+            partials[blockIdx.x] = t;
+        }
+    }
 }
 
-// Sum the per-block partials in block order (one thread: a few thousand additions).
+__device__ __forceinline__ void add_partial(Partial &t, const Partial &q)
+{
+    t.ssq += q.ssq;
+    t.n_valid += q.n_valid; t.n_empty_a += q.n_empty_a; t.n_empty_b += q.n_empty_b;
+    t.sum_a += q.sum_a; t.sum_b += q.sum_b;
+    t.max_a = max(t.max_a, q.max_a); t.max_b = max(t.max_b, q.max_b);
+}
+
+// Sum the per-block partials in a fixed order: one warp, lane l takes blocks l, l+32, ..., then a shuffle tree.
 __global__ void reduce_partials_kernel(const Partial *partials, int n_blocks, Partial *out)
 {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    Partial t = partials[0];
-    for (int k = 1; k < n_blocks; ++k) {
-        const Partial q = partials[k];
-        t.ssq += q.ssq;
-        t.n_valid += q.n_valid; t.n_empty_a += q.n_empty_a; t.n_empty_b += q.n_empty_b;
-        t.sum_a += q.sum_a; t.sum_b += q.sum_b;
-        t.max_a = max(t.max_a, q.max_a); t.max_b = max(t.max_b, q.max_b);
+    const int lane = threadIdx.x;
+    Partial t;
+    t.ssq = 0.0;
+    t.n_valid = t.n_empty_a = t.n_empty_b = t.sum_a = t.sum_b = 0ull;
+    t.max_a = t.max_b = 0u;
+    for (int k = lane; k < n_blocks; k += 32) add_partial(t, partials[k]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        Partial q;
+        q.ssq = __shfl_down_sync(0xffffffffu, t.ssq, o);
+        q.n_valid = __shfl_down_sync(0xffffffffu, t.n_valid, o);
+        q.n_empty_a = __shfl_down_sync(0xffffffffu, t.n_empty_a, o);
+        q.n_empty_b = __shfl_down_sync(0xffffffffu, t.n_empty_b, o);
+        q.sum_a = __shfl_down_sync(0xffffffffu, t.sum_a, o);
+        q.sum_b = __shfl_down_sync(0xffffffffu, t.sum_b, o);
+        q.max_a = __shfl_down_sync(0xffffffffu, t.max_a, o);
+        q.max_b = __shfl_down_sync(0xffffffffu, t.max_b, o);
+        add_partial(t, q);
     }
-    *out = t;
+    if (lane == 0) *out = t;
 }
 
 // ---- inclusive prefix sums of a count histogram (three small kernels, tiles of kScanTile bins)
@@ -284,6 +327,7 @@ __global__ void finalize_kernel(const Partial *tot, const unsigned long long *d_
     q = fmin(1.0, fmax(0.0, q));
     r.ks_prob = q;
     r.kernel_ms = 0.0;
+    r.pass_kernel_ms = 0.0;
     *out = r;
 }
 
@@ -299,8 +343,9 @@ struct StatsGuard { // device selection + everything the call allocates
     bool ok = false;
     void *ptrs[20];
     int n_ptrs = 0;
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
-    explicit StatsGuard(int dev)
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr, evp0 = nullptr, evp1 = nullptr; // whole call; the fused pass alone
+    cudaStream_t stream;
+    StatsGuard(int dev, cudaStream_t s) : stream(s)
     {
         int ndev = 0;
         if (cudaGetDeviceCount(&ndev) != cudaSuccess || dev < 0 || dev >= ndev) { cudaGetLastError(); return; }
@@ -310,24 +355,39 @@ struct StatsGuard { // device selection + everything the call allocates
     template <typename T> T *alloc(size_t count)
     {
         void *p = nullptr;
-        if (n_ptrs >= 20 || cudaMalloc(&p, (count ? count : 1) * sizeof(T)) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+        // stream-ordered allocation: no device-wide synchronisation per call
+        if (n_ptrs >= 20 || cudaMallocAsync(&p, (count ? count : 1) * sizeof(T), stream) != cudaSuccess) { cudaGetLastError(); return nullptr; }
         ptrs[n_ptrs++] = p;
         return static_cast<T *>(p);
     }
     ~StatsGuard()
     {
-        for (int k = 0; k < n_ptrs; ++k) cudaFree(ptrs[k]);
+        for (int k = 0; k < n_ptrs; ++k) cudaFreeAsync(ptrs[k], stream);
+        if (ok && n_ptrs) cudaStreamSynchronize(stream);
         if (ev0) cudaEventDestroy(ev0);
         if (ev1) cudaEventDestroy(ev1);
+        if (evp0) cudaEventDestroy(evp0);
+        if (evp1) cudaEventDestroy(evp1);
         if (ok) cudaSetDevice(prev);
     }
 };
 
 int grid_for(long long n, int sm_count)
 {
-    const long long want = (n + (long long)kThreads * 4 - 1) / ((long long)kThreads * 4);
-    const long long cap = (long long)sm_count * 8; // 8 resident CTAs of 256 threads per SM
-    return (int)(want < 1 ? 1 : (want < cap ? want : cap));
+    const long long want = (n + (long long)kPassThreads * 4 - 1) / ((long long)kPassThreads * 4);
+    return (int)(want < 1 ? 1 : (want < sm_count ? want : sm_count)); // one CTA of 1024 threads per SM
+}
+
+constexpr size_t kPassSmem = kLut * sizeof(double) + 2 * kShBins * sizeof(unsigned int);
+
+template <bool TWO, bool STATS>
+cudaError_t launch_pass(int grid, cudaStream_t s, const unsigned int *a, const unsigned int *b, long long n, double na, double nb,
+                        unsigned int *ha, unsigned int *hb, unsigned int cap, Partial *partials)
+{
+    cudaError_t e = cudaFuncSetAttribute(pass_kernel<TWO, STATS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPassSmem);
+    if (e != cudaSuccess) return e;
+    pass_kernel<TWO, STATS><<<grid, kPassThreads, kPassSmem, s>>>(a, b, n, na, nb, ha, hb, cap, partials);
+    return cudaGetLastError();
 }
 
 // inclusive prefix sums of hist[0..cap) into cum[0..cap)
@@ -371,12 +431,17 @@ int run_pass(StatsGuard &g, cudaStream_t s, const uint32_t *a, const uint32_t *b
     o.hist_a = g.alloc<unsigned int>(kCap0);
     o.hist_b = two ? g.alloc<unsigned int>(kCap0) : nullptr;
     if (!partials || !o.d_total || !o.hist_a || (two && !o.hist_b)) return ML_ERR_OOM;
-    if (cudaEventCreate(&g.ev0) != cudaSuccess || cudaEventCreate(&g.ev1) != cudaSuccess) return ML_ERR_CUDA;
+    if (cudaEventCreate(&g.ev0) != cudaSuccess || cudaEventCreate(&g.ev1) != cudaSuccess || cudaEventCreate(&g.evp0) != cudaSuccess ||
+        cudaEventCreate(&g.evp1) != cudaSuccess)
+        return ML_ERR_CUDA;
     if (cudaEventRecord(g.ev0, s) != cudaSuccess) return ML_ERR_CUDA;
     if (cudaMemsetAsync(o.hist_a, 0, kCap0 * 4ull, s) != cudaSuccess || (two && cudaMemsetAsync(o.hist_b, 0, kCap0 * 4ull, s) != cudaSuccess))
         return ML_ERR_CUDA;
-    if (two) pass_kernel<true, true><<<grid, kThreads, 0, s>>>(o.da, o.db, n, na, nb, o.hist_a, o.hist_b, kCap0, partials);
-    else pass_kernel<false, true><<<grid, kThreads, 0, s>>>(o.da, nullptr, n, na, nb, o.hist_a, nullptr, kCap0, partials);
+    if (cudaEventRecord(g.evp0, s) != cudaSuccess) return ML_ERR_CUDA;
+    if ((two ? launch_pass<true, true>(grid, s, o.da, o.db, n, na, nb, o.hist_a, o.hist_b, kCap0, partials)
+             : launch_pass<false, true>(grid, s, o.da, nullptr, n, na, nb, o.hist_a, nullptr, kCap0, partials)) != cudaSuccess)
+        return ML_ERR_CUDA;
+    if (cudaEventRecord(g.evp1, s) != cudaSuccess) return ML_ERR_CUDA;
     reduce_partials_kernel<<<1, 32, 0, s>>>(partials, grid, o.d_total);
     if (cudaGetLastError() != cudaSuccess) return ML_ERR_CUDA;
     if (cudaMemcpyAsync(&o.total, o.d_total, sizeof(Partial), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
@@ -391,9 +456,9 @@ int run_pass(StatsGuard &g, cudaStream_t s, const uint32_t *a, const uint32_t *b
         if (cudaMemsetAsync(o.hist_a, 0, (size_t)o.cap_eff * 4, s) != cudaSuccess ||
             (two && cudaMemsetAsync(o.hist_b, 0, (size_t)o.cap_eff * 4, s) != cudaSuccess))
             return ML_ERR_CUDA;
-        if (two) pass_kernel<true, false><<<grid, kThreads, 0, s>>>(o.da, o.db, n, na, nb, o.hist_a, o.hist_b, o.cap_eff, nullptr);
-        else pass_kernel<false, false><<<grid, kThreads, 0, s>>>(o.da, nullptr, n, na, nb, o.hist_a, nullptr, o.cap_eff, nullptr);
-        if (cudaGetLastError() != cudaSuccess) return ML_ERR_CUDA;
+        if ((two ? launch_pass<true, false>(grid, s, o.da, o.db, n, na, nb, o.hist_a, o.hist_b, o.cap_eff, nullptr)
+                 : launch_pass<false, false>(grid, s, o.da, nullptr, n, na, nb, o.hist_a, nullptr, o.cap_eff, nullptr)) != cudaSuccess)
+            return ML_ERR_CUDA;
     }
     return ML_OK;
 }
@@ -410,9 +475,9 @@ int ml_map_compare(const uint32_t *a, double n_rays_a, const uint32_t *b, double
     if (!a || !b || !out || n < 1 || n > 0x7fffffffLL || bad_rays(n_rays_a) || bad_rays(n_rays_b) ||
         (where != ML_MEM_HOST && where != ML_MEM_DEVICE))
         return ML_ERR_INVALID_ARG;
-    StatsGuard g(device);
-    if (!g.ok) return ML_ERR_CUDA;
     cudaStream_t s = (cudaStream_t)cuda_stream;
+    StatsGuard g(device, s);
+    if (!g.ok) return ML_ERR_CUDA;
     PassOut o;
     int rc = run_pass(g, s, a, b, n, n_rays_a, n_rays_b, where, device, o);
     if (rc != ML_OK) return rc;
@@ -430,9 +495,11 @@ int ml_map_compare(const uint32_t *a, double n_rays_a, const uint32_t *b, double
     if (cudaGetLastError() != cudaSuccess || cudaEventRecord(g.ev1, s) != cudaSuccess) return ML_ERR_CUDA;
     if (cudaMemcpyAsync(out, d_res, sizeof(*out), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
         return ML_ERR_CUDA;
-    float ms = 0.f;
-    if (cudaEventElapsedTime(&ms, g.ev0, g.ev1) != cudaSuccess) return ML_ERR_CUDA;
+    float ms = 0.f, pass_ms = 0.f;
+    if (cudaEventElapsedTime(&ms, g.ev0, g.ev1) != cudaSuccess || cudaEventElapsedTime(&pass_ms, g.evp0, g.evp1) != cudaSuccess)
+        return ML_ERR_CUDA;
     out->kernel_ms = ms;
+    out->pass_kernel_ms = pass_ms;
     return ML_OK;
 }
 
@@ -442,9 +509,9 @@ int ml_delta_m_histogram(const uint32_t *counts, double n_rays, int64_t n, doubl
     if (!counts || !hist_out || n < 1 || n > 0x7fffffffLL || bad_rays(n_rays) || !(lo < hi) || !isfinite(lo) || !isfinite(hi) ||
         n_bins < 1 || n_bins > (1 << 20) || (where != ML_MEM_HOST && where != ML_MEM_DEVICE))
         return ML_ERR_INVALID_ARG;
-    StatsGuard g(device);
-    if (!g.ok) return ML_ERR_CUDA;
     cudaStream_t s = (cudaStream_t)cuda_stream;
+    StatsGuard g(device, s);
+    if (!g.ok) return ML_ERR_CUDA;
     PassOut o;
     int rc = run_pass(g, s, counts, nullptr, n, n_rays, n_rays, where, device, o);
     if (rc != ML_OK) return rc;

@@ -3,7 +3,8 @@ eq. 10) against oracle/mapstats_oracle.py on the same seeded maps, through the C
 
 Bar: integer outputs (pixel counts, sums, maxima, histograms) bit-exact; the K-S distance is a difference of two
 integer ratios, compared to 1e-14 absolute; RMS (fp64 log10 of up to 1.7e7 pixels, fixed summation order on the
-device, numpy pairwise on the host) to 1e-12 relative; Q_KS to 1e-10.
+device, numpy pairwise on the host) to 1e-11 relative -- both sides form Delta m_a - Delta m_b from two rounded
+logarithms (absolute error <= ~2e-15 per pixel against differences of 1e-3 mag and more); Q_KS to 1e-10.
 """
 import numpy as np
 import pytest
@@ -36,7 +37,7 @@ def check(a, na, b, nb, **kw):
     assert r["n_empty_a"] == int((a_h == 0).sum()) and r["n_empty_b"] == int((b_h == 0).sum())
     rms, n_valid = mo.rms_delta_m(a_h, na, b_h, nb)
     assert r["n_valid"] == n_valid
-    assert abs(r["rms_delta_m"] - rms) <= 1e-12 * max(rms, 1e-300) + 1e-15, (r["rms_delta_m"], rms)
+    assert abs(r["rms_delta_m"] - rms) <= 1e-11 * max(rms, 1e-300) + 1e-15, (r["rms_delta_m"], rms)
     d = mo.ks_statistic(a_h, na, b_h, nb)
     assert abs(r["ks_d"] - d) <= 1e-14, (r["ks_d"], d)
     q = mo.ks_probability(d, a_h.size, b_h.size)
@@ -117,7 +118,7 @@ def test_device_pointers_on_real_maps_fp32_vs_fp64():
         r = ml.ml_map_compare(ml.ml_get_map_device(m32.ctx), p.n_rays, ml.ml_get_map_device(m64.ctx), p.n_rays, n=n)
         a, b = m32.counts(), m64.counts()
     rms, nv = mo.rms_delta_m(a, p.n_rays, b, p.n_rays)
-    assert r["n_valid"] == nv and abs(r["rms_delta_m"] - rms) <= 1e-12 * rms + 1e-15
+    assert r["n_valid"] == nv and abs(r["rms_delta_m"] - rms) <= 1e-11 * rms + 1e-15
     assert abs(r["ks_d"] - mo.ks_statistic(a, p.n_rays, b, p.n_rays)) <= 1e-14
     # "excellent agreement" in the paper's sense: RMS < 0.2 mag and P(KS) > 99.7 %
     assert r["rms_delta_m"] < 0.2 and r["ks_prob"] > 0.997
@@ -128,7 +129,7 @@ def test_device_pointers_on_real_maps_fp32_vs_fp64():
     s = torch.cuda.Stream()
     r2 = ml.ml_map_compare(ta.data_ptr() + 4, p.n_rays, tb.data_ptr() + 4, p.n_rays, n=n - 1, cuda_stream=s.cuda_stream)
     rms2, nv2 = mo.rms_delta_m(a.ravel()[1:], p.n_rays, b.ravel()[1:], p.n_rays)
-    assert r2["n_valid"] == nv2 and abs(r2["rms_delta_m"] - rms2) <= 1e-12 * rms2 + 1e-15
+    assert r2["n_valid"] == nv2 and abs(r2["rms_delta_m"] - rms2) <= 1e-11 * rms2 + 1e-15
 
 
 def test_argument_validation():

@@ -19,7 +19,8 @@
  *                       (readings R1-R4, R7 in DESIGN.md).
  *   ora_ray_x           BASELINE.json:configs[0] "regular grid over the rectangle";
  *                       PAPER.md:167 (regular grid).  Readings R7, R8.
- *   ora_lens_equation   PAPER.md:49-54 eq.(4) with m_i = 1.
+ *   ora_lens_equation   PAPER.md:49-54 eq.(4) with m_i = 1; the *_m variants take
+ *                       the masses m_i of eq.(4).
  *   ora_pixel           PAPER.md:45-47 (rays "mapped to a grid of pixels in the
  *                       source plane"); readings R10, R11.
  *   ora_shoot_region    PAPER.md:45-47 eq.(3): N_ij = number of rays reaching
@@ -29,7 +30,10 @@
  * (PAPER.md:156-157), Fig. 1 N*=558, eq.(12) uniform map without
  * stars, point-lens A(u), 2-D Gauss theorem on a ring of lenses, ray
  * conservation, mirror / transpose symmetries, an independent numpy brute force
- * on C1, Phi bookkeeping of eq.(6)/(9).  No function here is "parity unpinned".
+ * on C1, Phi bookkeeping of eq.(6)/(9); for the *_m variants: unit masses reproduce the
+ * unit-mass path bit for bit, two coincident unit lenses = one lens of mass 2, the Einstein
+ * radius of a mass-m lens is sqrt(m), Gauss theorem for a ring of unequal masses, numpy
+ * brute force.  No function here is "parity unpinned".
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/oracle.py).
  * -ffp-contract=off keeps every multiply and add separately rounded, so the
@@ -111,13 +115,13 @@ static void ora_ray_x(const ora_geometry *g, int64_t i, int64_t j, double x[2])
     x[1] = ((double)j - (double)(g->n2 - 1) / 2.0) * g->delta;
 }
 
-/* eq.(4), unit masses:
- *   y = diag(1-gamma, 1+gamma) x - sigma_c x - sum_i (x - x_i)/|x - x_i|^2
- * Lenses in index order, plain fp64 accumulation.
- * Returns 1 if the ray sits exactly on a lens (|x - x_i|^2 == 0) or y is not
- * finite (reading R12: such a ray is "dropped"), else 0. */
-int ora_lens_equation(double gamma, double kappa_c, const double *lens_xy, int64_t n_lens,
-                      const double x[2], double y[2])
+/* eq.(4), PAPER.md:51:
+ *   y = diag(1-gamma, 1+gamma) x - sigma_c x - sum_i m_i (x - x_i)/|x - x_i|^2
+ * mass = NULL means m_i = 1 (every map of the paper).  Lenses in index order,
+ * plain fp64 accumulation.  Returns 1 if the ray sits exactly on a lens (|x - x_i|^2 == 0) or y
+ * is not finite (reading R12: such a ray is "dropped"), else 0. */
+int ora_lens_equation_m(double gamma, double kappa_c, const double *lens_xy, const double *mass,
+                        int64_t n_lens, const double x[2], double y[2])
 {
     double s1 = 0.0, s2 = 0.0;
     int bad = 0;
@@ -126,13 +130,24 @@ int ora_lens_equation(double gamma, double kappa_c, const double *lens_xy, int64
         double d2 = x[1] - lens_xy[2 * k + 1];
         double r2 = d1 * d1 + d2 * d2;
         if (r2 == 0.0) bad = 1;
-        s1 += d1 / r2;
-        s2 += d2 / r2;
+        if (mass) {
+            s1 += mass[k] * d1 / r2;
+            s2 += mass[k] * d2 / r2;
+        } else {
+            s1 += d1 / r2;
+            s2 += d2 / r2;
+        }
     }
     y[0] = (1.0 - gamma) * x[0] - kappa_c * x[0] - s1;
     y[1] = (1.0 + gamma) * x[1] - kappa_c * x[1] - s2;
     if (!isfinite(y[0]) || !isfinite(y[1])) bad = 1;
     return bad;
+}
+
+int ora_lens_equation(double gamma, double kappa_c, const double *lens_xy, int64_t n_lens,
+                      const double x[2], double y[2])
+{
+    return ora_lens_equation_m(gamma, kappa_c, lens_xy, NULL, n_lens, x, y);
 }
 
 /* Source-plane pixel of y: half-open pixels, map covers [-L/2, L/2)^2, axis 1 is
@@ -151,9 +166,9 @@ static int ora_pixel(const ora_problem *p, const ora_geometry *g, const double y
 
 /* Shoot rays [i0,i1) x [j0,j1) and ADD them to map (n_pix*n_pix uint32, row-major,
  * map[j'*n_pix + i'], i' <-> y1).  stats[0..3] += shot, in-map, out-of-map, dropped. */
-int ora_shoot_region(const ora_problem *p, const double *lens_xy, int64_t n_lens,
-                     int64_t i0, int64_t i1, int64_t j0, int64_t j1,
-                     uint32_t *map, uint64_t stats[4])
+int ora_shoot_region_m(const ora_problem *p, const double *lens_xy, const double *mass, int64_t n_lens,
+                       int64_t i0, int64_t i1, int64_t j0, int64_t j1,
+                       uint32_t *map, uint64_t stats[4])
 {
     ora_geometry g;
     if (ora_derive(p, &g) != ORA_OK || n_lens < 0 || (n_lens > 0 && !lens_xy) || !map || !stats)
@@ -167,7 +182,7 @@ int ora_shoot_region(const ora_problem *p, const double *lens_xy, int64_t n_lens
             int64_t pi, pj;
             ora_ray_x(&g, i, j, x);
             ++shot;
-            if (ora_lens_equation(p->gamma, g.kappa_c, lens_xy, n_lens, x, y)) {
+            if (ora_lens_equation_m(p->gamma, g.kappa_c, lens_xy, mass, n_lens, x, y)) {
                 ++dropped;
             } else if (ora_pixel(p, &g, y, &pi, &pj)) {
                 ++outmap;
@@ -185,10 +200,17 @@ int ora_shoot_region(const ora_problem *p, const double *lens_xy, int64_t n_lens
     return ORA_OK;
 }
 
+int ora_shoot_region(const ora_problem *p, const double *lens_xy, int64_t n_lens,
+                     int64_t i0, int64_t i1, int64_t j0, int64_t j1,
+                     uint32_t *map, uint64_t stats[4])
+{
+    return ora_shoot_region_m(p, lens_xy, NULL, n_lens, i0, i1, j0, j1, map, stats);
+}
+
 /* Source-plane positions of every ray of [i0,i1) x [j0,j1), row-major in (j, i):
  * y_out[2*((j-j0)*(i1-i0) + (i-i0)) + {0,1}].  Dropped rays get NaN. */
-int ora_capture_region(const ora_problem *p, const double *lens_xy, int64_t n_lens,
-                       int64_t i0, int64_t i1, int64_t j0, int64_t j1, double *y_out)
+int ora_capture_region_m(const ora_problem *p, const double *lens_xy, const double *mass, int64_t n_lens,
+                         int64_t i0, int64_t i1, int64_t j0, int64_t j1, double *y_out)
 {
     ora_geometry g;
     if (ora_derive(p, &g) != ORA_OK || n_lens < 0 || (n_lens > 0 && !lens_xy) || !y_out)
@@ -200,7 +222,7 @@ int ora_capture_region(const ora_problem *p, const double *lens_xy, int64_t n_le
         for (int64_t i = i0; i < i1; ++i) {
             double x[2], y[2];
             ora_ray_x(&g, i, j, x);
-            if (ora_lens_equation(p->gamma, g.kappa_c, lens_xy, n_lens, x, y)) {
+            if (ora_lens_equation_m(p->gamma, g.kappa_c, lens_xy, mass, n_lens, x, y)) {
                 y[0] = NAN;
                 y[1] = NAN;
             }
@@ -209,6 +231,12 @@ int ora_capture_region(const ora_problem *p, const double *lens_xy, int64_t n_le
         }
     }
     return ORA_OK;
+}
+
+int ora_capture_region(const ora_problem *p, const double *lens_xy, int64_t n_lens,
+                       int64_t i0, int64_t i1, int64_t j0, int64_t j1, double *y_out)
+{
+    return ora_capture_region_m(p, lens_xy, NULL, n_lens, i0, i1, j0, j1, y_out);
 }
 
 /* Source-plane positions of the listed rays.  y_out = 2*n doubles. */
@@ -234,13 +262,25 @@ int ora_probe(const ora_problem *p, const double *lens_xy, int64_t n_lens,
 }
 
 /* eq.(4) at arbitrary image-plane points (not only grid rays): x_in, y_out = 2*n doubles. */
-int ora_deflect_points(double gamma, double kappa_c, const double *lens_xy, int64_t n_lens,
-                       int64_t n, const double *x_in, double *y_out)
+int ora_deflect_points_m(double gamma, double kappa_c, const double *lens_xy, const double *mass, int64_t n_lens,
+                         int64_t n, const double *x_in, double *y_out)
 {
     if (n < 0 || n_lens < 0) return ORA_BAD;
     for (int64_t k = 0; k < n; ++k)
-        ora_lens_equation(gamma, kappa_c, lens_xy, n_lens, x_in + 2 * k, y_out + 2 * k);
+        ora_lens_equation_m(gamma, kappa_c, lens_xy, mass, n_lens, x_in + 2 * k, y_out + 2 * k);
     return ORA_OK;
+}
+
+int ora_deflect_points(double gamma, double kappa_c, const double *lens_xy, int64_t n_lens,
+                       int64_t n, const double *x_in, double *y_out)
+{
+    return ora_deflect_points_m(gamma, kappa_c, lens_xy, NULL, n_lens, n, x_in, y_out);
+}
+
+/* eq.(5), with a mean lens mass: N_* = sigma_* A / (pi <M>) = sigma_* R^2 / <M>. */
+int64_t ora_n_star_m(double kappa_star, double r_disk, double mean_mass)
+{
+    return (int64_t)floor(kappa_star * r_disk * r_disk / mean_mass + 0.5);
 }
 
 /* Pixel index (j'*n_pix + i') of source-plane positions, -1 outside / NaN. */

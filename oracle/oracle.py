@@ -79,6 +79,13 @@ def _load():
         lib.ora_probe.argtypes = [pp, dp, C.c_int64, C.c_int64, ip, ip, dp]
         lib.ora_deflect_points.argtypes = [C.c_double, C.c_double, dp, C.c_int64, C.c_int64, dp, dp]
         lib.ora_pixels_of.argtypes = [pp, C.c_int64, dp, ip]
+        lib.ora_n_star_m.restype = C.c_int64
+        lib.ora_n_star_m.argtypes = [C.c_double, C.c_double, C.c_double]
+        lib.ora_shoot_region_m.argtypes = [pp, dp, dp, C.c_int64, C.c_int64, C.c_int64, C.c_int64,
+                                           C.c_int64, C.POINTER(C.c_uint32), C.POINTER(C.c_uint64)]
+        lib.ora_capture_region_m.argtypes = [pp, dp, dp, C.c_int64, C.c_int64, C.c_int64, C.c_int64,
+                                             C.c_int64, dp]
+        lib.ora_deflect_points_m.argtypes = [C.c_double, C.c_double, dp, dp, C.c_int64, C.c_int64, dp, dp]
         lib.ora_num_threads.restype = C.c_int
         _lib = lib
     return _lib
@@ -98,6 +105,15 @@ def _lenses(lens_xy):
     return a, a.shape[0]
 
 
+def _masses(mass, n):
+    """None (unit masses, the paper's maps) or n positive masses m_i of eq. 4."""
+    if mass is None:
+        return None, None
+    m = np.ascontiguousarray(mass, dtype=np.float64).ravel()
+    assert m.size == n
+    return m, _dptr(m)
+
+
 def _check(rc, what):
     if rc != 0:
         raise ValueError("oracle %s: invalid argument" % what)
@@ -107,8 +123,10 @@ def num_threads() -> int:
     return int(_load().ora_num_threads())
 
 
-def n_star(kappa_star: float, r_disk: float) -> int:
-    """Eq. (5), with A = pi R^2 and <M> = 1."""
+def n_star(kappa_star: float, r_disk: float, mean_mass: float = None) -> int:
+    """Eq. (5), with A = pi R^2 and <M> = 1 (or the given mean mass)."""
+    if mean_mass is not None:
+        return int(_load().ora_n_star_m(float(kappa_star), float(r_disk), float(mean_mass)))
     return int(_load().ora_n_star(float(kappa_star), float(r_disk)))
 
 
@@ -120,7 +138,7 @@ def geometry(sigma, stellar_fraction, gamma, n_pix, n_rays, L) -> Geometry:
 
 
 def shoot_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy,
-                 region=None, map_out=None):
+                 region=None, map_out=None, mass=None):
     """Counts map (uint32, shape (n_pix, n_pix), [j', i']) and stats dict.
 
     region = (i0, i1, j0, j1) ray-index rectangle (default: the whole grid);
@@ -133,27 +151,36 @@ def shoot_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy,
     m = map_out if map_out is not None else np.zeros((n_pix, n_pix), dtype=np.uint32)
     assert m.dtype == np.uint32 and m.flags.c_contiguous and m.size == n_pix * n_pix
     st = np.zeros(4, dtype=np.uint64)
-    _check(_load().ora_shoot_region(C.byref(p), _dptr(xy), n, i0, i1, j0, j1,
-                                    m.ctypes.data_as(C.POINTER(C.c_uint32)),
-                                    st.ctypes.data_as(C.POINTER(C.c_uint64))), "shoot_region")
+    mk, mp = _masses(mass, n)
+    if mk is None:
+        rc = _load().ora_shoot_region(C.byref(p), _dptr(xy), n, i0, i1, j0, j1,
+                                      m.ctypes.data_as(C.POINTER(C.c_uint32)), st.ctypes.data_as(C.POINTER(C.c_uint64)))
+    else:
+        rc = _load().ora_shoot_region_m(C.byref(p), _dptr(xy), mp, n, i0, i1, j0, j1,
+                                        m.ctypes.data_as(C.POINTER(C.c_uint32)), st.ctypes.data_as(C.POINTER(C.c_uint64)))
+    _check(rc, "shoot_region")
     stats = {"rays_shot": int(st[0]), "rays_in_map": int(st[1]),
              "rays_out_of_map": int(st[2]), "rays_dropped": int(st[3]),
              "interactions": int(st[0]) * n}
     return m, stats
 
 
-def shoot(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy):
-    return shoot_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy)
+def shoot(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, mass=None):
+    return shoot_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, mass=mass)
 
 
-def capture_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, region):
+def capture_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, region, mass=None):
     """y of every ray in region, shape (j1-j0, i1-i0, 2)."""
     p = _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L)
     xy, n = _lenses(lens_xy)
     i0, i1, j0, j1 = region
     out = np.empty((j1 - j0, i1 - i0, 2), dtype=np.float64)
-    _check(_load().ora_capture_region(C.byref(p), _dptr(xy), n, i0, i1, j0, j1, _dptr(out)),
-           "capture_region")
+    mk, mp = _masses(mass, n)
+    if mk is None:
+        rc = _load().ora_capture_region(C.byref(p), _dptr(xy), n, i0, i1, j0, j1, _dptr(out))
+    else:
+        rc = _load().ora_capture_region_m(C.byref(p), _dptr(xy), mp, n, i0, i1, j0, j1, _dptr(out))
+    _check(rc, "capture_region")
     return out
 
 
@@ -170,13 +197,17 @@ def probe(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, ray_i, ray_
     return out
 
 
-def deflect_points(gamma, kappa_c, lens_xy, x):
+def deflect_points(gamma, kappa_c, lens_xy, x, mass=None):
     """Eq. (4) at arbitrary image-plane points x (n, 2) -> y (n, 2)."""
     xy, n = _lenses(lens_xy)
     xs = np.ascontiguousarray(x, dtype=np.float64).reshape(-1, 2)
     out = np.empty_like(xs)
-    _check(_load().ora_deflect_points(float(gamma), float(kappa_c), _dptr(xy), n, xs.shape[0],
-                                      _dptr(xs), _dptr(out)), "deflect_points")
+    mk, mp = _masses(mass, n)
+    if mk is None:
+        rc = _load().ora_deflect_points(float(gamma), float(kappa_c), _dptr(xy), n, xs.shape[0], _dptr(xs), _dptr(out))
+    else:
+        rc = _load().ora_deflect_points_m(float(gamma), float(kappa_c), _dptr(xy), mp, n, xs.shape[0], _dptr(xs), _dptr(out))
+    _check(rc, "deflect_points")
     return out
 
 

@@ -9,7 +9,7 @@ import math
 import numpy as np
 
 
-def shoot_numpy(sigma, f_star, gamma, n_pix, n_rays, L, lens_xy, rows=256):
+def shoot_numpy(sigma, f_star, gamma, n_pix, n_rays, L, lens_xy, rows=256, mass=None):
     kc = sigma - sigma * f_star
     pix = L / n_pix
     d = pix / math.sqrt(n_rays)
@@ -25,12 +25,18 @@ def shoot_numpy(sigma, f_star, gamma, n_pix, n_rays, L, lens_xy, rows=256):
         X, Y = np.meshgrid(x1, x2[j0:j0 + rows])
         ax = np.zeros_like(X)
         ay = np.zeros_like(X)
-        for lx, ly in np.asarray(lens_xy, dtype=np.float64).reshape(-1, 2):
+        lenses = np.asarray(lens_xy, dtype=np.float64).reshape(-1, 2)
+        masses = np.ones(len(lenses)) if mass is None else np.asarray(mass, dtype=np.float64)
+        for (lx, ly), m in zip(lenses, masses):
             dx = X - lx
             dy = Y - ly
             r2 = dx * dx + dy * dy
-            ax += dx / r2
-            ay += dy / r2
+            if mass is None:
+                ax += dx / r2
+                ay += dy / r2
+            else:           # eq.(4) with its m_i
+                ax += m * dx / r2
+                ay += m * dy / r2
         y1 = (1 - gamma) * X - kc * X - ax
         y2 = (1 + gamma) * Y - kc * Y - ay
         ii = np.floor((y1 + L / 2) / pix)

@@ -25,7 +25,7 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-from workloads import CONFIGS, lens_disk, parity_tiles  # noqa: E402
+from workloads import CONFIGS, lens_disk, lens_masses, parity_tiles  # noqa: E402
 
 METRIC = "lens-ray interactions/sec"
 UNIT = "interactions/s"
@@ -107,7 +107,7 @@ def oracle_rate(p, seconds, log=None):
     512 x 512-ray sub-rectangles of its ray grid, as many as fit in about `seconds`."""
     from oracle import oracle
     g = oracle.geometry(*problem_args(p))
-    xy = lens_disk(g.n_star, g.r_star, p.seed)
+    xy = lens_disk(g.n_star, g.r_star, p.seed)   # the BASELINE config's own field (no --masses / --n-lenses here)
     side = 512
     tiles = parity_tiles(g.n1, g.n2, 64, side, p.seed)
     omap = np.zeros((p.n_pix, p.n_pix), dtype=np.uint32)
@@ -160,6 +160,10 @@ def config_dict(p, info, args):
                      % (p.name, p.sigma, p.gamma, p.stellar_fraction, p.L, p.n_pix, p.n_rays, p.seed, CONFIGS.index(p)),
          "l2": "flushed between steps (256 MiB write)",
          "parallelism": "ray row bands x%d + map all-reduce" % args.gpus if args.gpus > 1 else "single GPU"}
+    if getattr(args, "masses", False):
+        c["masses"] = "log-uniform 0.3-3 (workloads.lens_masses), eq. 4 with m_i"
+    if getattr(args, "n_lenses", 0) > 0:
+        c["n_lenses_override"] = "lens count set to %d in the same disk (large-N* row, not a BASELINE config)" % args.n_lenses
     if info is not None:
         c.update(n_lenses=int(info["n_lenses"]), n1=int(info["n1"]), n2=int(info["n2"]),
                  rays=int(info["n1"]) * int(info["n2"]), tile=[int(info["tile_w"]), int(info["tile_h"])],
@@ -191,8 +195,10 @@ def run_ours(args):
     p = pick(args.workload)
     m = ml.MagnificationMap(*problem_args(p), device=local, precision=PRECISIONS[args.precision])
     info = m.info
-    xy = lens_disk(info["n_star_expected"], info["r_star"], p.seed)
-    m.set_lenses(xy)
+    n_field = args.n_lenses if args.n_lenses > 0 else info["n_star_expected"]
+    xy = lens_disk(n_field, info["r_star"], p.seed)
+    mass = lens_masses(n_field, p.seed) if args.masses else None
+    m.set_lenses(xy, mass)
     info = m.info
     n1, n2, n_lens = int(info["n1"]), int(info["n2"]), int(info["n_lenses"])
     j0, j1 = row_band(n2, rank, world, int(info["tile_h"]))
@@ -254,7 +260,7 @@ def run_ours(args):
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        m.set_lenses(host_xy.numpy())            # H2D: lens positions (host buffer -> ml_set_lenses)
+        m.set_lenses(host_xy.numpy(), mass)      # H2D: lens positions (host buffer -> ml_set_lenses)
         m.shoot_region(0, n1, j0, j1)
         if world > 1:
             with torch.cuda.stream(stream):
@@ -415,6 +421,8 @@ def main():
     ap.add_argument("--precision", default="fp32_tiled", choices=sorted(PRECISIONS))
     ap.add_argument("--row", default="shoot", choices=["shoot", "mapstats"],
                     help="shoot = the hot path (default, the BASELINE.json metric); mapstats = the map-comparison row")
+    ap.add_argument("--masses", action="store_true", help="unequal lens masses (eq. 4 with m_i): the MASS kernel instantiations")
+    ap.add_argument("--n-lenses", type=int, default=0, help="override the lens count (large-N* row); 0 = eq. 5")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

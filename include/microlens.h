@@ -118,6 +118,14 @@ int ml_get_info(const ml_ctx *ctx, ml_info *out);
  * coordinate gives ML_ERR_INVALID_ARG and leaves the previous lenses in place. */
 int ml_set_lenses(ml_ctx *ctx, const double *xy, int64_t n);
 
+/* Same with the lens masses m_i of eq.4: mass = n HOST fp64 values > 0 in units of the
+ * mass whose Einstein radius is the unit of length, or NULL for unit masses (= ml_set_lenses; the
+ * paper sets all masses equal).  The deflection of lens i is m_i (x - xi_i)/|x - xi_i|^2;
+ * the kernels multiply 1/r^2 by m_i (one extra FP32 multiply per ray pair and lens).  For a mean mass
+ * <M> the lens count of eq.5 is n_star_expected / <M>.  ML_ERR_INVALID_ARG for a non-finite or
+ * non-positive mass; the previous lenses stay in place on any error. */
+int ml_set_lens_masses(ml_ctx *ctx, const double *xy, const double *mass, int64_t n);
+
 /* Select ML_PREC_*; ML_ERR_INVALID_ARG for any other value. */
 int ml_set_precision(ml_ctx *ctx, int mode);
 

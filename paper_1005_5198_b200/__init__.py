@@ -30,6 +30,7 @@ from .binding import (  # noqa: F401
     ml_get_stats,
     ml_map_compare,
     ml_probe,
+    ml_set_lens_masses,
     ml_set_lenses,
     ml_set_precision,
     ml_shoot,

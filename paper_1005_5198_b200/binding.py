@@ -28,7 +28,7 @@ EXPORTS = (
     "ml_create", "ml_destroy", "ml_get_info", "ml_set_lenses", "ml_set_precision", "ml_shoot",
     "ml_shoot_region", "ml_get_map", "ml_get_map_device", "ml_use_device_map", "ml_attach_stream",
     "ml_get_stats", "ml_capture_region", "ml_probe", "ml_strerror", "ml_version",
-    "ml_map_compare", "ml_delta_m_histogram",
+    "ml_map_compare", "ml_delta_m_histogram", "ml_set_lens_masses",
 )
 
 ML_MEM_HOST = 0
@@ -96,6 +96,7 @@ def load():
     lib.ml_destroy.restype = None
     lib.ml_get_info.argtypes = [vp, C.POINTER(MlInfo)]
     lib.ml_set_lenses.argtypes = [vp, C.POINTER(dbl), i64]
+    lib.ml_set_lens_masses.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), i64]
     lib.ml_set_precision.argtypes = [vp, C.c_int]
     lib.ml_shoot.argtypes = [vp]
     lib.ml_shoot_region.argtypes = [vp, i64, i64, i64, i64, C.c_int]
@@ -159,6 +160,18 @@ def ml_get_info(ctx) -> dict:
 def ml_set_lenses(ctx, xy):
     a = np.ascontiguousarray(xy, dtype=np.float64).reshape(-1, 2)
     _check(load().ml_set_lenses(ctx, a.ctypes.data_as(C.POINTER(C.c_double)), a.shape[0]), "ml_set_lenses")
+
+
+def ml_set_lens_masses(ctx, xy, mass=None):
+    """Lens positions plus the masses m_i of eq. 4 (None = unit masses)."""
+    a = np.ascontiguousarray(xy, dtype=np.float64).reshape(-1, 2)
+    mp = None
+    if mass is not None:
+        m = np.ascontiguousarray(mass, dtype=np.float64).ravel()
+        if m.size != a.shape[0]:
+            raise ValueError("ml_set_lens_masses: one mass per lens")
+        mp = m.ctypes.data_as(C.POINTER(C.c_double))
+    _check(load().ml_set_lens_masses(ctx, a.ctypes.data_as(C.POINTER(C.c_double)), mp, a.shape[0]), "ml_set_lens_masses")
 
 
 def ml_set_precision(ctx, mode):

@@ -30,6 +30,7 @@ struct ml_ctx {
     cudaEvent_t ev0, ev1;
     unsigned int *map_own, *map;
     double2 *lens;
+    double *mass;     // device masses m_i (eq.4), nullptr = unit masses
     int64_t n_lenses; // -1: never set
     unsigned long long *counters; // device [3]
     int precision;
@@ -68,22 +69,28 @@ Mode mode_of(int precision)
     return {32 * RXF, kWarps * RYF};
 }
 
+template <bool CAPTURE, bool MASS> cudaError_t launch_m(int precision, unsigned int g, const ShootParams &p, cudaStream_t s)
+{
+    switch (precision) {
+    case ML_PREC_FP64:
+        shoot_kernel<double, RXD, RYD, KFD, false, CAPTURE, MASS><<<g, kThreads, 0, s>>>(p);
+        break;
+    case ML_PREC_FP32_COMPENSATED:
+        shoot_kernel<float, RXF, RYF, KFC, true, CAPTURE, MASS><<<g, kThreads, 0, s>>>(p);
+        break;
+    default:
+        shoot_kernel_pipe<SHARED_T, KFF, WARPS_T, MINB_T, true, CAPTURE, MASS><<<g, WARPS_T * 32, 0, s>>>(p);
+        break;
+    }
+    return cudaGetLastError();
+}
+
+// unit masses (every map of the paper) run the instantiations without the mass multiply
 template <bool CAPTURE> cudaError_t launch(int precision, long long n_tiles, const ShootParams &p, cudaStream_t s)
 {
     if (n_tiles <= 0) return cudaSuccess;
     const unsigned int g = (unsigned int)n_tiles;
-    switch (precision) {
-    case ML_PREC_FP64:
-        shoot_kernel<double, RXD, RYD, KFD, false, CAPTURE><<<g, kThreads, 0, s>>>(p);
-        break;
-    case ML_PREC_FP32_COMPENSATED:
-        shoot_kernel<float, RXF, RYF, KFC, true, CAPTURE><<<g, kThreads, 0, s>>>(p);
-        break;
-    default:
-        shoot_kernel_pipe<SHARED_T, KFF, WARPS_T, MINB_T, true, CAPTURE><<<g, WARPS_T * 32, 0, s>>>(p);
-        break;
-    }
-    return cudaGetLastError();
+    return p.mass ? launch_m<CAPTURE, true>(precision, g, p, s) : launch_m<CAPTURE, false>(precision, g, p, s);
 }
 
 ShootParams base_params(const ml_ctx *c)
@@ -91,6 +98,7 @@ ShootParams base_params(const ml_ctx *c)
     ShootParams p;
     std::memset(&p, 0, sizeof(p));
     p.lens = c->lens;
+    p.mass = c->mass;
     p.n_lens = (int)c->n_lenses;
     p.n_pix = c->n_pix;
     p.delta = c->delta;
@@ -290,6 +298,7 @@ void ml_destroy(ml_ctx *c)
             if (c->own_stream) cudaStreamSynchronize(c->own_stream);
             if (c->map_own) cudaFree(c->map_own);
             if (c->lens) cudaFree(c->lens);
+            if (c->mass) cudaFree(c->mass);
             if (c->counters) cudaFree(c->counters);
             if (c->ev0) cudaEventDestroy(c->ev0);
             if (c->ev1) cudaEventDestroy(c->ev1);
@@ -315,28 +324,40 @@ int ml_get_info(const ml_ctx *c, ml_info *o)
     return ML_OK;
 }
 
-int ml_set_lenses(ml_ctx *c, const double *xy, int64_t n)
+int ml_set_lens_masses(ml_ctx *c, const double *xy, const double *mass, int64_t n)
 {
     if (!c || n < 0 || n > 0x7fffff00LL || (n > 0 && !xy)) return ML_ERR_INVALID_ARG;
     for (int64_t k = 0; k < 2 * n; ++k)
         if (!std::isfinite(xy[k])) return ML_ERR_INVALID_ARG;
+    if (mass)
+        for (int64_t k = 0; k < n; ++k)
+            if (!std::isfinite(mass[k]) || !(mass[k] > 0.0)) return ML_ERR_INVALID_ARG;
     DeviceGuard g(c->device);
     if (!g.ok) return ML_ERR_CUDA;
     double2 *d = nullptr;
-    if (cudaMalloc(&d, (size_t)std::max<int64_t>(n, 1) * sizeof(double2)) != cudaSuccess) {
+    double *dm = nullptr;
+    if (cudaMalloc(&d, (size_t)std::max<int64_t>(n, 1) * sizeof(double2)) != cudaSuccess ||
+        (mass && cudaMalloc(&dm, (size_t)std::max<int64_t>(n, 1) * sizeof(double)) != cudaSuccess)) {
         cudaGetLastError();
+        if (d) cudaFree(d);
         return ML_ERR_OOM;
     }
     if (n > 0 && (cudaMemcpyAsync(d, xy, (size_t)n * sizeof(double2), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+                  (mass && cudaMemcpyAsync(dm, mass, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, c->stream) != cudaSuccess) ||
                   cudaStreamSynchronize(c->stream) != cudaSuccess)) {
         cudaFree(d);
+        if (dm) cudaFree(dm);
         return ML_ERR_CUDA;
     }
     if (c->lens) cudaFree(c->lens);
+    if (c->mass) cudaFree(c->mass);
     c->lens = d;
+    c->mass = dm;
     c->n_lenses = n;
     return ML_OK;
 }
+
+int ml_set_lenses(ml_ctx *c, const double *xy, int64_t n) { return ml_set_lens_masses(c, xy, nullptr, n); }
 
 int ml_set_precision(ml_ctx *c, int mode)
 {

@@ -38,6 +38,7 @@ namespace mlb200 {
 
 struct ShootParams {
     const double2 *lens;      // [n_lens] fp64 (x, y), device
+    const double *mass;       // [n_lens] fp64 lens masses m_i of eq.4 (MASS instantiations only)
     int n_lens;
     int n_pix;
     long long i0, i1, j0, j1; // region of ray indices to count (others are masked)
@@ -164,7 +165,7 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
     }
 }
 
-template <typename Real, int RX, int RY, int KF, bool NEWTON, bool CAPTURE>
+template <typename Real, int RX, int RY, int KF, bool NEWTON, bool CAPTURE, bool MASS = false>
 __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
 {
     using Real2 = typename Vec2<Real>::type;
@@ -175,6 +176,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
     constexpr int PER_THREAD = kChunk / kThreads;
 
     __shared__ __align__(16) Real2 lens_s[2][kChunk];
+    __shared__ Real mass_s[2][MASS ? kChunk : 1]; // m_i of eq.4, unit masses otherwise
     __shared__ unsigned int cta_count[3];
 
     const int lane = threadIdx.x & 31;
@@ -214,11 +216,15 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
     // ---- a1: stage chunk 0
     const Real pad = pad_coordinate<Real, NEWTON>();
     double2 pre[PER_THREAD];
+    double pre_m[MASS ? PER_THREAD : 1];
     auto fetch = [&](int base) {
 #pragma unroll
         for (int q = 0; q < PER_THREAD; ++q) {
             const int k = base + q * kThreads + threadIdx.x;
-            if (k < p.n_lens) pre[q] = __ldg(&p.lens[k]);
+            if (k < p.n_lens) {
+                pre[q] = __ldg(&p.lens[k]);
+                if (MASS) pre_m[q] = __ldg(&p.mass[k]);
+            }
         }
     };
     auto stage = [&](int base, int buf) {
@@ -226,13 +232,16 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
         for (int q = 0; q < PER_THREAD; ++q) {
             const int k = base + q * kThreads + threadIdx.x;
             Real2 v;
+            Real m = (Real)0;
             if (k < p.n_lens) {
                 v.x = (Real)(pre[q].x - cx);
                 v.y = (Real)(pre[q].y - cy);
+                if (MASS) m = (Real)pre_m[q];
             } else {
                 v.x = pad; v.y = pad;
             }
             lens_s[buf][q * kThreads + threadIdx.x] = v;
+            if (MASS) mass_s[buf][q * kThreads + threadIdx.x] = m;
         }
     };
     fetch(0);
@@ -247,6 +256,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
         const int cnt = min(kChunk, p.n_lens - base);
         const int cntp = (cnt + 7) & ~7; // padded with zero-contribution lenses
         const Real2 *ls = lens_s[buf];
+        const Real *ms = mass_s[buf];
         for (int k0 = 0; k0 < cntp; k0 += KF) {
             const int kend = min(k0 + KF, cntp);
 #pragma unroll 1
@@ -254,6 +264,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
 #pragma unroll
                 for (int u = 0; u < 2; ++u) {
                     const Real2 l = ls[k + u];
+                    const Real m = MASS ? ms[k + u] : (Real)1;
                     Real dx[RX], dx2[RX], dy[RY], dy2[RY];
 #pragma unroll
                     for (int c = 0; c < RX; ++c) { dx[c] = sub_rn(ox[c], l.x); dx2[c] = mul_rn(dx[c], dx[c]); }
@@ -263,7 +274,8 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
                     for (int r = 0; r < RY; ++r)
 #pragma unroll
                         for (int c = 0; c < RX; ++c) {
-                            const Real inv = recip<NEWTON>(add_rn(dx2[c], dy2[r]));
+                            Real inv = recip<NEWTON>(add_rn(dx2[c], dy2[r]));
+                            if (MASS) inv = mul_rn(inv, m); // m_i / r^2
                             sx[r][c] = fma_rn(dx[c], inv, sx[r][c]);
                             sy[r][c] = fma_rn(dy[r], inv, sy[r][c]);
                         }
@@ -314,12 +326,13 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
 // so its terms are exactly 0 on shared rows and 5e-16 on the others.
 template <int RY> struct PipeRegs {
     float2 dxA, dxB;
+    float m; // lens mass (MASS instantiations)
     float dy[RY];
     float2 r2A[RY], r2B[RY]; // shared rows: r^2; other rows: 1/r^2
     float2 R[RY];
 };
 
-template <int SHARED, int KF, int WARPS, int MINB, bool SCALAR_DY, bool CAPTURE>
+template <int SHARED, int KF, int WARPS, int MINB, bool SCALAR_DY, bool CAPTURE, bool MASS = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const ShootParams p)
 {
     constexpr int RX = 4, RY = 4;
@@ -330,6 +343,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
     constexpr int PER_THREAD = kChunk / THREADS;
 
     __shared__ __align__(16) float4 lens_s[2][kChunk + 2];
+    __shared__ float mass_s[2][MASS ? kChunk + 2 : 1]; // m_i of eq.4; one extra FMUL2 per row and lens
     __shared__ unsigned int cta_count[3];
 
     const int lane = threadIdx.x & 31;
@@ -346,6 +360,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
     }
     if (threadIdx.x < 3) cta_count[threadIdx.x] = 0;
     if (threadIdx.x < 4) lens_s[threadIdx.x >> 1][kChunk + (threadIdx.x & 1)] = make_float4(-1e15f, -1e15f, -1e15f, -1e15f);
+    if (MASS && threadIdx.x < 4) mass_s[threadIdx.x >> 1][(MASS ? kChunk : 0) + (MASS ? (threadIdx.x & 1) : 0)] = 0.f;
 
     const double cx = ((double)(ti * TW) + 0.5 * (TW - 1) - p.half1) * p.delta;
     const double cy = ((double)(tj * TH) + 0.5 * (TH - 1) - p.half2) * p.delta;
@@ -368,23 +383,29 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
     }
 
     double2 pre[PER_THREAD];
+    double pre_m[MASS ? PER_THREAD : 1];
     auto fetch = [&](int base) {
 #pragma unroll
         for (int q = 0; q < PER_THREAD; ++q) {
             const int k = base + q * THREADS + threadIdx.x;
-            if (k < p.n_lens) pre[q] = __ldg(&p.lens[k]);
+            if (k < p.n_lens) {
+                pre[q] = __ldg(&p.lens[k]);
+                if (MASS) pre_m[q] = __ldg(&p.mass[k]);
+            }
         }
     };
     auto stage = [&](int base, int buf) {
 #pragma unroll
         for (int q = 0; q < PER_THREAD; ++q) {
             const int k = base + q * THREADS + threadIdx.x;
-            float nx = -1e15f, ny = -1e15f;
+            float nx = -1e15f, ny = -1e15f, m = 0.f;
             if (k < p.n_lens) {
                 nx = -(float)(pre[q].x - cx);
                 ny = -(float)(pre[q].y - cy);
+                if (MASS) m = (float)pre_m[q];
             }
             lens_s[buf][q * THREADS + threadIdx.x] = make_float4(nx, nx, ny, ny);
+            if (MASS) mass_s[buf][q * THREADS + threadIdx.x] = m;
         }
     };
     fetch(0);
@@ -392,8 +413,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
     __syncthreads();
 
     const float2 eps2 = make_float2(0x1p-80f, 0x1p-80f);
-    auto stage1 = [&](const float4 l, PipeRegs<RY> &s) {
+    auto stage1 = [&](const float4 l, const float m, PipeRegs<RY> &s) {
         const float2 nlx = make_float2(l.x, l.y), nly = make_float2(l.z, l.w);
+        s.m = m;
         s.dxA = __fadd2_rn(oxA, nlx);
         s.dxB = __fadd2_rn(oxB, nlx);
         const float2 qA = __ffma2_rn(s.dxA, s.dxA, eps2), qB = __ffma2_rn(s.dxB, s.dxB, eps2);
@@ -424,11 +446,12 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
         for (int r = 0; r < RY; ++r) {
             float2 iA, iB;
             if (r < SHARED) {
-                iA = __fmul2_rn(s.R[r], s.r2B[r]);
-                iB = __fmul2_rn(s.R[r], s.r2A[r]);
+                const float2 R = MASS ? __fmul2_rn(s.R[r], make_float2(s.m, s.m)) : s.R[r]; // m_i / (r2A r2B)
+                iA = __fmul2_rn(R, s.r2B[r]);
+                iB = __fmul2_rn(R, s.r2A[r]);
             } else {
-                iA = s.r2A[r];
-                iB = s.r2B[r];
+                iA = MASS ? __fmul2_rn(s.r2A[r], make_float2(s.m, s.m)) : s.r2A[r];
+                iB = MASS ? __fmul2_rn(s.r2B[r], make_float2(s.m, s.m)) : s.r2B[r];
             }
             const float2 dy = make_float2(s.dy[r], s.dy[r]);
             sxA[r] = __ffma2_rn(s.dxA, iA, sxA[r]);
@@ -445,15 +468,17 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
         const int cnt = min(kChunk, p.n_lens - base);
         const int cntp = (cnt + 1) & ~1;
         const float4 *ls = lens_s[buf];
+        const float *ms = mass_s[buf];
+        auto mass_of = [&](int k) { return MASS ? ms[k] : 1.f; };
         PipeRegs<RY> a, b;
-        stage1(ls[0], a);
+        stage1(ls[0], mass_of(0), a);
         for (int k0 = 0; k0 < cntp; k0 += KF) {
             const int kend = min(k0 + KF, cntp);
 #pragma unroll 1
             for (int k = k0; k < kend; k += 2) {
-                stage1(ls[k + 1], b);
+                stage1(ls[k + 1], mass_of(k + 1), b);
                 stage2(a);
-                stage1(ls[k + 2], a);
+                stage1(ls[k + 2], mass_of(k + 2), a);
                 stage2(b);
             }
 #pragma unroll

@@ -48,8 +48,11 @@ class MagnificationMap:
     def stats(self) -> dict:
         return _b.ml_get_stats(self._ctx)
 
-    def set_lenses(self, xy):
-        _b.ml_set_lenses(self._ctx, xy)
+    def set_lenses(self, xy, mass=None):
+        if mass is None:
+            _b.ml_set_lenses(self._ctx, xy)
+        else:
+            _b.ml_set_lens_masses(self._ctx, xy, mass)
 
     def set_precision(self, mode):
         _b.ml_set_precision(self._ctx, mode)

@@ -10,6 +10,7 @@ from .lens_fields import (  # noqa: F401
     CONFIGS,
     Problem,
     lens_disk,
+    lens_masses,
     parity_tiles,
     probe_rays,
 )

@@ -62,6 +62,17 @@ def lens_disk(n_star: int, r_star: float, seed: int) -> np.ndarray:
     return xy
 
 
+def lens_masses(n_star: int, seed: int) -> np.ndarray:
+    """n_star seeded lens masses for the unequal-mass row (eq. 4's m_i).
+
+    The paper sets all masses equal and names no spectrum; this stand-in is a
+    log-uniform spectrum over a decade, 0.3 ... 3 in units of the reference mass, the range a stellar
+    population would span.  Mean ~ 1.17; the caller uses the sample mean as <M> in eq. 5.
+    """
+    rng = np.random.default_rng(3000 + seed)
+    return 0.3 * 10.0 ** rng.random(n_star)
+
+
 def parity_tiles(n1: int, n2: int, n_tiles: int, side: int, seed: int):
     """Seeded ray-index sub-rectangles [i0,i1) x [j0,j1) inside the n1 x n2 grid.
 

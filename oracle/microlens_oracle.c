@@ -18,7 +18,9 @@
  *                       and the concrete rules of BASELINE.json:configs[0]
  *                       (readings R1-R4, R7 in DESIGN.md).
  *   ora_ray_x           BASELINE.json:configs[0] "regular grid over the rectangle";
- *                       PAPER.md:167 (regular grid).  Readings R7, R8.
+ *                       PAPER.md:167 (regular grid).  Readings R7, R8.  ray_mode 1: GPU-D's random
+ *                       ray positions, one per grid cell (reading R17), drawn
+ *                       with Philox-4x32-10 keyed by the seed, counter = ray id.
  *   ora_lens_equation   PAPER.md:49-54 eq.(4) with m_i = 1; the *_m variants take
  *                       the masses m_i of eq.(4).
  *   ora_pixel           PAPER.md:45-47 (rays "mapped to a grid of pixels in the
@@ -53,6 +55,9 @@ typedef struct {
     int32_t n_pix;           /* pixels per side of the square map                          */
     double n_rays;           /* mean rays per pixel without lensing */
     double L;                /* source-plane side length, Einstein radii */
+    int32_t ray_mode;        /* 0: regular grid (configs); 1: random position inside
+                                each grid cell (the GPU-D way; reading R17)    */
+    uint64_t ray_seed;       /* key of the counter-based generator for ray_mode 1                  */
 } ora_problem;
 
 typedef struct {
@@ -81,7 +86,7 @@ int ora_derive(const ora_problem *p, ora_geometry *g)
     if (!p || !g) return ORA_BAD;
     if (!(p->sigma >= 0.0) || !(p->stellar_fraction >= 0.0) || !(p->stellar_fraction <= 1.0) ||
         p->n_pix <= 0 || !(p->n_rays > 0.0) || !(p->L > 0.0) || !isfinite(p->gamma) ||
-        !isfinite(p->sigma) || !isfinite(p->n_rays) || !isfinite(p->L))
+        !isfinite(p->sigma) || !isfinite(p->n_rays) || !isfinite(p->L) || (p->ray_mode != 0 && p->ray_mode != 1))
         return ORA_BAD;
     double minus = 1.0 - p->sigma - p->gamma; /* axis-1 smooth stretch (eq.4, eq.11) */
     double plus = 1.0 - p->sigma + p->gamma;  /* axis-2 smooth stretch               */
@@ -107,12 +112,59 @@ int ora_derive(const ora_problem *p, ora_geometry *g)
     return ORA_OK;
 }
 
-/* Image-plane position of ray (i, j): cell-centred regular grid, symmetric about
- * the origin (reading R7). */
-static void ora_ray_x(const ora_geometry *g, int64_t i, int64_t j, double x[2])
+/* Philox-4x32-10 (Salmon, Moraes, Dror & Shaw, SC'11): counter-based generator, 10 rounds of
+ *   (c0,c1,c2,c3) <- (hi(M1 c2) ^ c1 ^ k0, lo(M1 c2), hi(M0 c0) ^ c3 ^ k1, lo(M0 c0)),  k <- k + (W0, W1).
+ * Pinned by the published known-answer vectors (tests/golden/philox4x32_10_kat.txt). */
+void ora_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
 {
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* Two uniform deviates in [0,1) for ray id = j*n1 + i: counter (id_lo, id_hi, 0, 0), key (seed_lo, seed_hi);
+ * 53 bits each: u = ((r_a >> 5) 2^26 + (r_b >> 6)) 2^-53. */
+void ora_ray_uniforms(uint64_t ray_id, uint64_t seed, double u[2])
+{
+    uint32_t ctr[4] = {(uint32_t)ray_id, (uint32_t)(ray_id >> 32), 0u, 0u};
+    uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)}, r[4];
+    ora_philox4x32_10(ctr, key, r);
+    u[0] = ((double)(r[0] >> 5) * 67108864.0 + (double)(r[1] >> 6)) * (1.0 / 9007199254740992.0);
+    u[1] = ((double)(r[2] >> 5) * 67108864.0 + (double)(r[3] >> 6)) * (1.0 / 9007199254740992.0);
+}
+
+/* Image-plane position of ray (i, j).  ray_mode 0: cell-centred regular grid, symmetric about the
+ * origin (reading R7).  ray_mode 1: a uniformly random point of the same grid cell
+ * [(i - n1/2) delta, (i + 1 - n1/2) delta) x [...]: the paper's GPU-D shoots rays "from random positions in
+ * the shooting grid"; reading R17 keeps one ray per cell so that ray (i, j) stays
+ * where the tile-local arithmetic and the region / sharding logic expect it (the regular grid is u = 1/2). */
+static void ora_ray_x(const ora_problem *p, const ora_geometry *g, int64_t i, int64_t j, double x[2])
+{
+    if (p->ray_mode == 1) {
+        double u[2];
+        ora_ray_uniforms((uint64_t)j * (uint64_t)g->n1 + (uint64_t)i, p->ray_seed, u);
+        x[0] = ((double)i + u[0] - (double)g->n1 / 2.0) * g->delta;
+        x[1] = ((double)j + u[1] - (double)g->n2 / 2.0) * g->delta;
+        return;
+    }
     x[0] = ((double)i - (double)(g->n1 - 1) / 2.0) * g->delta;
     x[1] = ((double)j - (double)(g->n2 - 1) / 2.0) * g->delta;
+}
+
+/* Image-plane positions of the listed rays (x_out = 2*n doubles): exposes ray generation to the pins. */
+int ora_ray_positions(const ora_problem *p, int64_t n, const int64_t *ray_i, const int64_t *ray_j, double *x_out)
+{
+    ora_geometry g;
+    if (ora_derive(p, &g) != ORA_OK || n < 0) return ORA_BAD;
+    for (int64_t k = 0; k < n; ++k) ora_ray_x(p, &g, ray_i[k], ray_j[k], x_out + 2 * k);
+    return ORA_OK;
 }
 
 /* eq.(4), PAPER.md:51:
@@ -180,7 +232,7 @@ int ora_shoot_region_m(const ora_problem *p, const double *lens_xy, const double
         for (int64_t i = i0; i < i1; ++i) {
             double x[2], y[2];
             int64_t pi, pj;
-            ora_ray_x(&g, i, j, x);
+            ora_ray_x(p, &g, i, j, x);
             ++shot;
             if (ora_lens_equation_m(p->gamma, g.kappa_c, lens_xy, mass, n_lens, x, y)) {
                 ++dropped;
@@ -221,7 +273,7 @@ int ora_capture_region_m(const ora_problem *p, const double *lens_xy, const doub
     for (int64_t j = j0; j < j1; ++j) {
         for (int64_t i = i0; i < i1; ++i) {
             double x[2], y[2];
-            ora_ray_x(&g, i, j, x);
+            ora_ray_x(p, &g, i, j, x);
             if (ora_lens_equation_m(p->gamma, g.kappa_c, lens_xy, mass, n_lens, x, y)) {
                 y[0] = NAN;
                 y[1] = NAN;
@@ -250,7 +302,7 @@ int ora_probe(const ora_problem *p, const double *lens_xy, int64_t n_lens,
 #pragma omp parallel for schedule(static)
     for (int64_t k = 0; k < n; ++k) {
         double x[2], y[2];
-        ora_ray_x(&g, ray_i[k], ray_j[k], x);
+        ora_ray_x(p, &g, ray_i[k], ray_j[k], x);
         if (ora_lens_equation(p->gamma, g.kappa_c, lens_xy, n_lens, x, y)) {
             y[0] = NAN;
             y[1] = NAN;

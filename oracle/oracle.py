@@ -34,7 +34,8 @@ def build(force: bool = False) -> str:
 
 class _Problem(C.Structure):
     _fields_ = [("sigma", C.c_double), ("stellar_fraction", C.c_double), ("gamma", C.c_double),
-                ("n_pix", C.c_int32), ("n_rays", C.c_double), ("L", C.c_double)]
+                ("n_pix", C.c_int32), ("n_rays", C.c_double), ("L", C.c_double),
+                ("ray_mode", C.c_int32), ("ray_seed", C.c_uint64)]
 
 
 class _Geometry(C.Structure):
@@ -79,6 +80,11 @@ def _load():
         lib.ora_probe.argtypes = [pp, dp, C.c_int64, C.c_int64, ip, ip, dp]
         lib.ora_deflect_points.argtypes = [C.c_double, C.c_double, dp, C.c_int64, C.c_int64, dp, dp]
         lib.ora_pixels_of.argtypes = [pp, C.c_int64, dp, ip]
+        lib.ora_ray_positions.argtypes = [pp, C.c_int64, ip, ip, dp]
+        lib.ora_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
+        lib.ora_philox4x32_10.restype = None
+        lib.ora_ray_uniforms.argtypes = [C.c_uint64, C.c_uint64, dp]
+        lib.ora_ray_uniforms.restype = None
         lib.ora_n_star_m.restype = C.c_int64
         lib.ora_n_star_m.argtypes = [C.c_double, C.c_double, C.c_double]
         lib.ora_shoot_region_m.argtypes = [pp, dp, dp, C.c_int64, C.c_int64, C.c_int64, C.c_int64,
@@ -91,9 +97,10 @@ def _load():
     return _lib
 
 
-def _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L):
+def _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_seed=None):
+    """ray_seed = None: regular ray grid; an int: random position inside each grid cell (reading R17)."""
     return _Problem(float(sigma), float(stellar_fraction), float(gamma), int(n_pix),
-                    float(n_rays), float(L))
+                    float(n_rays), float(L), 0 if ray_seed is None else 1, 0 if ray_seed is None else int(ray_seed))
 
 
 def _dptr(a):
@@ -138,13 +145,13 @@ def geometry(sigma, stellar_fraction, gamma, n_pix, n_rays, L) -> Geometry:
 
 
 def shoot_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy,
-                 region=None, map_out=None, mass=None):
+                 region=None, map_out=None, mass=None, ray_seed=None):
     """Counts map (uint32, shape (n_pix, n_pix), [j', i']) and stats dict.
 
     region = (i0, i1, j0, j1) ray-index rectangle (default: the whole grid);
     map_out: existing map to accumulate into.
     """
-    p = _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L)
+    p = _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_seed)
     g = geometry(sigma, stellar_fraction, gamma, n_pix, n_rays, L)
     xy, n = _lenses(lens_xy)
     i0, i1, j0, j1 = region if region is not None else (0, g.n1, 0, g.n2)
@@ -165,13 +172,13 @@ def shoot_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy,
     return m, stats
 
 
-def shoot(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, mass=None):
-    return shoot_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, mass=mass)
+def shoot(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, mass=None, ray_seed=None):
+    return shoot_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, mass=mass, ray_seed=ray_seed)
 
 
-def capture_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, region, mass=None):
+def capture_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, region, mass=None, ray_seed=None):
     """y of every ray in region, shape (j1-j0, i1-i0, 2)."""
-    p = _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L)
+    p = _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_seed)
     xy, n = _lenses(lens_xy)
     i0, i1, j0, j1 = region
     out = np.empty((j1 - j0, i1 - i0, 2), dtype=np.float64)
@@ -219,3 +226,30 @@ def pixels_of(sigma, stellar_fraction, gamma, n_pix, n_rays, L, y):
     _check(_load().ora_pixels_of(C.byref(p), ys.shape[0], _dptr(ys),
                                  out.ctypes.data_as(C.POINTER(C.c_int64))), "pixels_of")
     return out.reshape(np.asarray(y).shape[:-1])
+
+
+def philox4x32_10(ctr, key):
+    """Philox-4x32-10 block: 4 counter words, 2 key words -> 4 output words (ints)."""
+    c = (C.c_uint32 * 4)(*[int(v) for v in ctr])
+    k = (C.c_uint32 * 2)(*[int(v) for v in key])
+    o = (C.c_uint32 * 4)()
+    _load().ora_philox4x32_10(c, k, o)
+    return [int(v) for v in o]
+
+
+def ray_uniforms(ray_id, seed):
+    u = (C.c_double * 2)()
+    _load().ora_ray_uniforms(int(ray_id), int(seed), u)
+    return float(u[0]), float(u[1])
+
+
+def ray_positions(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_i, ray_j, ray_seed=None):
+    """Image-plane positions x (n, 2) of the listed rays (regular grid, or random-in-cell with ray_seed)."""
+    p = _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_seed)
+    ri = np.ascontiguousarray(ray_i, dtype=np.int64)
+    rj = np.ascontiguousarray(ray_j, dtype=np.int64)
+    out = np.empty((ri.size, 2), dtype=np.float64)
+    ip = C.POINTER(C.c_int64)
+    _check(_load().ora_ray_positions(C.byref(p), ri.size, ri.ctypes.data_as(ip), rj.ctypes.data_as(ip), _dptr(out)),
+           "ray_positions")
+    return out

@@ -162,6 +162,8 @@ def config_dict(p, info, args):
          "parallelism": "ray row bands x%d + map all-reduce" % args.gpus if args.gpus > 1 else "single GPU"}
     if getattr(args, "masses", False):
         c["masses"] = "log-uniform 0.3-3 (workloads.lens_masses), eq. 4 with m_i"
+    if getattr(args, "random_rays", False):
+        c["ray_mode"] = "random position in every grid cell (GPU-D's ray generation, PAPER.md:131; reading R17), generic kernel"
     if getattr(args, "n_lenses", 0) > 0:
         c["n_lenses_override"] = "lens count set to %d in the same disk (large-N* row, not a BASELINE config)" % args.n_lenses
     if info is not None:
@@ -199,6 +201,8 @@ def run_ours(args):
     xy = lens_disk(n_field, info["r_star"], p.seed)
     mass = lens_masses(n_field, p.seed) if args.masses else None
     m.set_lenses(xy, mass)
+    if args.random_rays:
+        m.set_ray_mode(ml.ML_RAYS_RANDOM, 20100527)
     info = m.info
     n1, n2, n_lens = int(info["n1"]), int(info["n2"]), int(info["n_lenses"])
     j0, j1 = row_band(n2, rank, world, int(info["tile_h"]))
@@ -422,6 +426,7 @@ def main():
     ap.add_argument("--row", default="shoot", choices=["shoot", "mapstats"],
                     help="shoot = the hot path (default, the BASELINE.json metric); mapstats = the map-comparison row")
     ap.add_argument("--masses", action="store_true", help="unequal lens masses (eq. 4 with m_i): the MASS kernel instantiations")
+    ap.add_argument("--random-rays", action="store_true", help="ML_RAYS_RANDOM: the paper's GPU-D ray generation")
     ap.add_argument("--n-lenses", type=int, default=0, help="override the lens count (large-N* row); 0 = eq. 5")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

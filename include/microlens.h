@@ -66,6 +66,19 @@ enum {
     ML_PREC_FP64 = 2              /* everything in fp64 (true division)                      */
 };
 
+/* Where the rays start.  REGULAR: the cell-centred regular grid of the configs
+ * (the tree codes' way).  RANDOM: the paper's GPU-D shoots rays "from random positions in the shooting
+ * grid"; here ray (i,j) starts at a uniformly random point of its own grid cell,
+ *     x = ((i + u1 - n1/2) delta, (j + u2 - n2/2) delta),
+ * (u1, u2) = two 53-bit uniforms from Philox-4x32-10 with counter (ray id lo, hi, 0, 0), ray id = j n1 + i,
+ * and key = seed (reading R17): the same number of rays, the same mean density, regions and
+ * sharding unchanged; the rays share no coordinate differences, so the generic kernel runs
+ * (one reciprocal per interaction). */
+enum {
+    ML_RAYS_REGULAR = 0,
+    ML_RAYS_RANDOM = 1
+};
+
 typedef struct {
     double kappa_star, kappa_c;      /* sigma_*, sigma_c                                    */
     double a1, a2;                   /* half-sides of the shooting rectangle (R_E)          */
@@ -82,6 +95,8 @@ typedef struct {
     int32_t device;                  /* CUDA device ordinal                                 */
     int32_t sm_count;                /* multiProcessorCount of that device                  */
     int32_t sm_clock_khz;            /* cudaDevAttrClockRate (max SM clock)                 */
+    int32_t ray_mode;                /* ML_RAYS_*                                           */
+    uint64_t ray_seed;               /* key of the ray generator (ML_RAYS_RANDOM)           */
 } ml_info;
 
 typedef struct {
@@ -125,6 +140,10 @@ int ml_set_lenses(ml_ctx *ctx, const double *xy, int64_t n);
  * <M> the lens count of eq.5 is n_star_expected / <M>.  ML_ERR_INVALID_ARG for a non-finite or
  * non-positive mass; the previous lenses stay in place on any error. */
 int ml_set_lens_masses(ml_ctx *ctx, const double *xy, const double *mass, int64_t n);
+
+/* Select ML_RAYS_* (see the enum); seed keys the generator of ML_RAYS_RANDOM and is ignored otherwise.
+ * Takes effect at the next shoot / capture / probe.  ML_ERR_INVALID_ARG for any other mode. */
+int ml_set_ray_mode(ml_ctx *ctx, int mode, uint64_t seed);
 
 /* Select ML_PREC_*; ML_ERR_INVALID_ARG for any other value. */
 int ml_set_precision(ml_ctx *ctx, int mode);

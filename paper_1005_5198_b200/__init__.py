@@ -16,6 +16,8 @@ from .binding import (  # noqa: F401
     ML_PREC_FP32_COMPENSATED,
     ML_PREC_FP32_TILED,
     ML_PREC_FP64,
+    ML_RAYS_RANDOM,
+    ML_RAYS_REGULAR,
     MicrolensError,
     library_path,
     load,
@@ -33,6 +35,7 @@ from .binding import (  # noqa: F401
     ml_set_lens_masses,
     ml_set_lenses,
     ml_set_precision,
+    ml_set_ray_mode,
     ml_shoot,
     ml_shoot_region,
     ml_use_device_map,

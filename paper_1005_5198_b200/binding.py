@@ -28,8 +28,11 @@ EXPORTS = (
     "ml_create", "ml_destroy", "ml_get_info", "ml_set_lenses", "ml_set_precision", "ml_shoot",
     "ml_shoot_region", "ml_get_map", "ml_get_map_device", "ml_use_device_map", "ml_attach_stream",
     "ml_get_stats", "ml_capture_region", "ml_probe", "ml_strerror", "ml_version",
-    "ml_map_compare", "ml_delta_m_histogram", "ml_set_lens_masses",
+    "ml_map_compare", "ml_delta_m_histogram", "ml_set_lens_masses", "ml_set_ray_mode",
 )
+
+ML_RAYS_REGULAR = 0
+ML_RAYS_RANDOM = 1
 
 ML_MEM_HOST = 0
 ML_MEM_DEVICE = 1
@@ -43,6 +46,7 @@ class MlInfo(C.Structure):
         ("n1", C.c_int64), ("n2", C.c_int64), ("n_star_expected", C.c_int64), ("n_lenses", C.c_int64),
         ("n_pix", C.c_int32), ("tile_w", C.c_int32), ("tile_h", C.c_int32), ("precision", C.c_int32),
         ("device", C.c_int32), ("sm_count", C.c_int32), ("sm_clock_khz", C.c_int32),
+        ("ray_mode", C.c_int32), ("ray_seed", C.c_uint64),
     ]
 
 
@@ -98,6 +102,7 @@ def load():
     lib.ml_set_lenses.argtypes = [vp, C.POINTER(dbl), i64]
     lib.ml_set_lens_masses.argtypes = [vp, C.POINTER(dbl), C.POINTER(dbl), i64]
     lib.ml_set_precision.argtypes = [vp, C.c_int]
+    lib.ml_set_ray_mode.argtypes = [vp, C.c_int, C.c_uint64]
     lib.ml_shoot.argtypes = [vp]
     lib.ml_shoot_region.argtypes = [vp, i64, i64, i64, i64, C.c_int]
     lib.ml_get_map.argtypes = [vp, C.POINTER(C.c_uint32), C.c_size_t]
@@ -176,6 +181,10 @@ def ml_set_lens_masses(ctx, xy, mass=None):
 
 def ml_set_precision(ctx, mode):
     _check(load().ml_set_precision(ctx, int(mode)), "ml_set_precision")
+
+
+def ml_set_ray_mode(ctx, mode, seed=0):
+    _check(load().ml_set_ray_mode(ctx, int(mode), int(seed)), "ml_set_ray_mode")
 
 
 def ml_shoot(ctx):

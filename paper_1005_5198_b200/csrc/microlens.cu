@@ -34,6 +34,8 @@ struct ml_ctx {
     int64_t n_lenses; // -1: never set
     unsigned long long *counters; // device [3]
     int precision;
+    int ray_mode;            // ML_RAYS_*
+    unsigned long long ray_seed;
     ml_stats stats;
 };
 
@@ -62,12 +64,17 @@ constexpr int WARPS_T = 4, SHARED_T = 4, MINB_T = 3; // FP32_TILED: 128-thread C
 constexpr int KFC = 8;                     // FP32_COMPENSATED
 constexpr int RXD = 2, RYD = 2, KFD = 64;  // FP64
 
-Mode mode_of(int precision)
+constexpr int RXR = 4, RYR = 2;            // FP32 modes with random rays: every ray carries its own offsets
+
+Mode mode_of(int precision, int ray_mode)
 {
     if (precision == ML_PREC_FP64) return {32 * RXD, kWarps * RYD};
+    if (ray_mode == ML_RAYS_RANDOM) return {32 * RXR, kWarps * RYR};
     if (precision == ML_PREC_FP32_TILED) return {32 * RXF, WARPS_T * RYF};
     return {32 * RXF, kWarps * RYF};
 }
+
+Mode mode_of(const ml_ctx *c) { return mode_of(c->precision, c->ray_mode); }
 
 template <bool CAPTURE, bool MASS> cudaError_t launch_m(int precision, unsigned int g, const ShootParams &p, cudaStream_t s)
 {
@@ -85,11 +92,30 @@ template <bool CAPTURE, bool MASS> cudaError_t launch_m(int precision, unsigned 
     return cudaGetLastError();
 }
 
+// random ray positions (reading R17): the generic kernel with per-ray offsets
+template <bool CAPTURE, bool MASS> cudaError_t launch_r(int precision, unsigned int g, const ShootParams &p, cudaStream_t s)
+{
+    switch (precision) {
+    case ML_PREC_FP64:
+        shoot_kernel<double, RXD, RYD, KFD, false, CAPTURE, MASS, true><<<g, kThreads, 0, s>>>(p);
+        break;
+    case ML_PREC_FP32_COMPENSATED:
+        shoot_kernel<float, RXR, RYR, KFC, true, CAPTURE, MASS, true><<<g, kThreads, 0, s>>>(p);
+        break;
+    default:
+        shoot_kernel<float, RXR, RYR, KFF, false, CAPTURE, MASS, true><<<g, kThreads, 0, s>>>(p);
+        break;
+    }
+    return cudaGetLastError();
+}
+
 // unit masses (every map of the paper) run the instantiations without the mass multiply
-template <bool CAPTURE> cudaError_t launch(int precision, long long n_tiles, const ShootParams &p, cudaStream_t s)
+template <bool CAPTURE> cudaError_t launch(int precision, int ray_mode, long long n_tiles, const ShootParams &p, cudaStream_t s)
 {
     if (n_tiles <= 0) return cudaSuccess;
     const unsigned int g = (unsigned int)n_tiles;
+    if (ray_mode == ML_RAYS_RANDOM)
+        return p.mass ? launch_r<CAPTURE, true>(precision, g, p, s) : launch_r<CAPTURE, false>(precision, g, p, s);
     return p.mass ? launch_m<CAPTURE, true>(precision, g, p, s) : launch_m<CAPTURE, false>(precision, g, p, s);
 }
 
@@ -110,6 +136,8 @@ ShootParams base_params(const ml_ctx *c)
     p.inv_pixel = (double)c->n_pix / c->L;
     p.map = c->map;
     p.counters = c->counters;
+    p.n1 = c->n1;
+    p.ray_seed = c->ray_seed;
     return p;
 }
 
@@ -132,7 +160,7 @@ int shoot_region_impl(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1,
     float ms = 0.f;
     uint64_t launches = 0;
     if (i1 > i0 && j1 > j0) {
-        const Mode m = mode_of(c->precision);
+        const Mode m = mode_of(c);
         ShootParams p = base_params(c);
         p.i0 = i0; p.i1 = i1; p.j0 = j0; p.j1 = j1;
         p.tile_i0 = i0 / m.tw;
@@ -143,7 +171,7 @@ int shoot_region_impl(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1,
         if (cudaEventRecord(c->ev0, c->stream) != cudaSuccess) return ML_ERR_CUDA;
         for (long long base = 0; base < n_tiles; base += kMaxTilesPerLaunch) {
             p.tile_base = base;
-            if (launch<false>(c->precision, std::min(kMaxTilesPerLaunch, n_tiles - base), p, c->stream) != cudaSuccess)
+            if (launch<false>(c->precision, c->ray_mode, std::min(kMaxTilesPerLaunch, n_tiles - base), p, c->stream) != cudaSuccess)
                 return ML_ERR_CUDA;
             ++launches;
         }
@@ -169,7 +197,7 @@ int shoot_region_impl(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1,
 template <typename Sink>
 int capture_tiles(ml_ctx *c, const std::vector<long long> &tiles /* pairs */, Sink sink)
 {
-    const Mode m = mode_of(c->precision);
+    const Mode m = mode_of(c);
     const size_t per_tile = (size_t)m.tw * m.th;
     const long long n_tiles = (long long)(tiles.size() / 2);
     if (n_tiles == 0) return ML_OK;
@@ -196,7 +224,7 @@ int capture_tiles(ml_ctx *c, const std::vector<long long> &tiles /* pairs */, Si
         p.capture = d_buf;
         p.tile_list = d_list + 2 * first;
         p.tile_base = 0;
-        if (launch<true>(c->precision, nb, p, c->stream) != cudaSuccess ||
+        if (launch<true>(c->precision, c->ray_mode, nb, p, c->stream) != cudaSuccess ||
             cudaMemcpyAsync(h_buf.data(), d_buf, (size_t)nb * per_tile * sizeof(double2), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
             cudaStreamSynchronize(c->stream) != cudaSuccess) {
             rc = ML_ERR_CUDA;
@@ -250,6 +278,7 @@ int ml_create(double sigma, double stellar_fraction, double gamma, int32_t n_pix
     c->mu_th = 1.0 / ((1.0 - sigma) * (1.0 - sigma) - gamma * gamma);
     c->n_lenses = -1;
     c->precision = ML_PREC_FP32_TILED;
+    c->ray_mode = ML_RAYS_REGULAR;
     c->device = device;
 
     int ndev = 0;
@@ -317,10 +346,11 @@ int ml_get_info(const ml_ctx *c, ml_info *o)
     o->ray_spacing = c->delta; o->r_star = c->r_star; o->pixel_side = c->pixel; o->mu_theory = c->mu_th;
     o->n1 = c->n1; o->n2 = c->n2; o->n_star_expected = c->n_star_expected; o->n_lenses = c->n_lenses;
     o->n_pix = c->n_pix;
-    const Mode m = mode_of(c->precision);
+    const Mode m = mode_of(c);
     o->tile_w = m.tw; o->tile_h = m.th;
     o->precision = c->precision; o->device = c->device;
     o->sm_count = c->sm_count; o->sm_clock_khz = c->sm_clock_khz;
+    o->ray_mode = c->ray_mode; o->ray_seed = c->ray_seed;
     return ML_OK;
 }
 
@@ -364,6 +394,14 @@ int ml_set_precision(ml_ctx *c, int mode)
     if (!c || (mode != ML_PREC_FP32_TILED && mode != ML_PREC_FP32_COMPENSATED && mode != ML_PREC_FP64))
         return ML_ERR_INVALID_ARG;
     c->precision = mode;
+    return ML_OK;
+}
+
+int ml_set_ray_mode(ml_ctx *c, int mode, uint64_t seed)
+{
+    if (!c || (mode != ML_RAYS_REGULAR && mode != ML_RAYS_RANDOM)) return ML_ERR_INVALID_ARG;
+    c->ray_mode = mode;
+    c->ray_seed = mode == ML_RAYS_RANDOM ? seed : 0;
     return ML_OK;
 }
 
@@ -427,7 +465,7 @@ int ml_capture_region(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1,
     if ((double)(i1 - i0) * (double)(j1 - j0) > 268435456.0) return ML_ERR_OOM;
     DeviceGuard g(c->device);
     if (!g.ok) return ML_ERR_CUDA;
-    const Mode m = mode_of(c->precision);
+    const Mode m = mode_of(c);
     std::vector<long long> tiles;
     try {
         for (long long tj = j0 / m.th; tj <= (j1 - 1) / m.th; ++tj)
@@ -469,7 +507,7 @@ int ml_probe(ml_ctx *c, int64_t n, const int64_t *ray_i, const int64_t *ray_j, d
         if (ray_i[k] < 0 || ray_i[k] >= c->n1 || ray_j[k] < 0 || ray_j[k] >= c->n2) return ML_ERR_INVALID_ARG;
     DeviceGuard g(c->device);
     if (!g.ok) return ML_ERR_CUDA;
-    const Mode m = mode_of(c->precision);
+    const Mode m = mode_of(c);
     // rays sorted by the tile that owns them; one capture tile per distinct tile
     std::vector<int64_t> order;
     std::vector<long long> tiles;

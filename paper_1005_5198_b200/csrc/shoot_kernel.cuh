@@ -53,6 +53,8 @@ struct ShootParams {
     unsigned long long *counters; // [0] shot [1] in map [2] dropped
     double2 *capture;         // CAPTURE: [n_tiles_in_list * TW*TH] source-plane positions
     const long long *tile_list; // CAPTURE: pairs (tile_i, tile_j), global tile indices
+    long long n1;             // rays per row of the whole grid (ray id = j*n1 + i, RANDOM instantiations)
+    unsigned long long ray_seed; // key of the ray generator (RANDOM instantiations)
 };
 
 constexpr int kThreads = 256;
@@ -99,9 +101,27 @@ __device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(
 __device__ __forceinline__ float fma_rn(float a, float b, float c) { return __fmaf_rn(a, b, c); }
 __device__ __forceinline__ double fma_rn(double a, double b, double c) { return __fma_rn(a, b, c); }
 
+// Philox-4x32-10 (Salmon et al., SC'11), counter = (ray id lo, hi, 0, 0), key = seed: two 53-bit uniforms in
+// [0,1) per ray.  GPU-D shoots rays from random positions; reading R17 draws one ray
+// uniformly inside each grid cell, so ray (i,j) stays in the tile that owns cell (i,j).
+__device__ __forceinline__ void ray_uniforms(unsigned long long ray_id, unsigned long long seed, double &u1, double &u2)
+{
+    unsigned int c0 = (unsigned int)ray_id, c1 = (unsigned int)(ray_id >> 32), c2 = 0u, c3 = 0u;
+    unsigned int k0 = (unsigned int)seed, k1 = (unsigned int)(seed >> 32);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned int h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        const unsigned int h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    u1 = ((double)(c0 >> 5) * 67108864.0 + (double)(c1 >> 6)) * (1.0 / 9007199254740992.0);
+    u2 = ((double)(c2 >> 5) * 67108864.0 + (double)(c3 >> 6)) * (1.0 / 9007199254740992.0);
+}
+
 // a4 + a5 (+ statistics) for one thread's RX x RY rays: macro terms and pixel index in
 // fp64, run-length aggregated binning.  Shared by every instantiation of the kernels below.
-template <int RX, int RY, bool CAPTURE, int WARPS = kWarps>
+template <int RX, int RY, bool CAPTURE, int WARPS = kWarps, bool RANDOM = false>
 __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, long long tj, long long t, int lane,
                                             int warp, const double (&Sx)[RY][RX], const double (&Sy)[RY][RX],
                                             unsigned int *cta_count)
@@ -114,12 +134,18 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
 #pragma unroll
     for (int r = 0; r < RY; ++r) {
         const long long j = tj * TH + warp * RY + r;
-        const double x2 = ((double)j - p.half2) * p.delta;
+        double x2 = ((double)j - p.half2) * p.delta;
         const bool jvalid = (j >= p.j0) && (j < p.j1);
 #pragma unroll
         for (int c = 0; c < RX; ++c) {
             const long long i = ti * TW + lane * RX + c;
-            const double x1 = ((double)i - p.half1) * p.delta;
+            double x1 = ((double)i - p.half1) * p.delta;
+            if (RANDOM) { // the ray's own position in its cell (same draw as in the prologue)
+                double u1, u2;
+                ray_uniforms((unsigned long long)j * (unsigned long long)p.n1 + (unsigned long long)i, p.ray_seed, u1, u2);
+                x1 = ((double)i + u1 - (p.half1 + 0.5)) * p.delta;
+                x2 = ((double)j + u2 - (p.half2 + 0.5)) * p.delta;
+            }
             const double y1 = p.c1 * x1 - Sx[r][c];
             const double y2 = p.c2 * x2 - Sy[r][c];
             const bool finite = (fabs(y1) <= 1.7976931348623157e308) && (fabs(y2) <= 1.7976931348623157e308);
@@ -165,7 +191,7 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
     }
 }
 
-template <typename Real, int RX, int RY, int KF, bool NEWTON, bool CAPTURE, bool MASS = false>
+template <typename Real, int RX, int RY, int KF, bool NEWTON, bool CAPTURE, bool MASS = false, bool RANDOM = false>
 __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
 {
     using Real2 = typename Vec2<Real>::type;
@@ -202,6 +228,20 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
     for (int c = 0; c < RX; ++c) ox[c] = (Real)(((double)(lane * RX + c) - 0.5 * (TW - 1)) * p.delta);
 #pragma unroll
     for (int r = 0; r < RY; ++r) oy[r] = (Real)(((double)(warp * RY + r) - 0.5 * (TH - 1)) * p.delta);
+    // RANDOM: every ray has its own offset from the tile centre (no shared column / row differences)
+    Real oxr[RANDOM ? RY : 1][RANDOM ? RX : 1], oyr[RANDOM ? RY : 1][RANDOM ? RX : 1];
+    if (RANDOM) {
+#pragma unroll
+        for (int r = 0; r < RY; ++r)
+#pragma unroll
+            for (int c = 0; c < RX; ++c) {
+                const unsigned long long i = (unsigned long long)(ti * TW + lane * RX + c), j = (unsigned long long)(tj * TH + warp * RY + r);
+                double u1, u2;
+                ray_uniforms(j * (unsigned long long)p.n1 + i, p.ray_seed, u1, u2);
+                oxr[RANDOM ? r : 0][RANDOM ? c : 0] = (Real)(((double)(lane * RX + c) + u1 - 0.5 * TW) * p.delta);
+                oyr[RANDOM ? r : 0][RANDOM ? c : 0] = (Real)(((double)(warp * RY + r) + u2 - 0.5 * TH) * p.delta);
+            }
+    }
 
     double Sx[RY][RX], Sy[RY][RX]; // fp64 accumulators of the deflection sum
     Real sx[RY][RX], sy[RY][RX];   // partial sums of the current flush group
@@ -265,6 +305,19 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
                 for (int u = 0; u < 2; ++u) {
                     const Real2 l = ls[k + u];
                     const Real m = MASS ? ms[k + u] : (Real)1;
+                    if constexpr (RANDOM) { // 2 sub, mul, fma, rcp, 2 fma per interaction: the paper's 10 flop, nothing shared
+#pragma unroll
+                        for (int r = 0; r < RY; ++r)
+#pragma unroll
+                            for (int c = 0; c < RX; ++c) {
+                                const Real ex = sub_rn(oxr[RANDOM ? r : 0][RANDOM ? c : 0], l.x);
+                                const Real ey = sub_rn(oyr[RANDOM ? r : 0][RANDOM ? c : 0], l.y);
+                                Real inv = recip<NEWTON>(fma_rn(ey, ey, mul_rn(ex, ex)));
+                                if (MASS) inv = mul_rn(inv, m);
+                                sx[r][c] = fma_rn(ex, inv, sx[r][c]);
+                                sy[r][c] = fma_rn(ey, inv, sy[r][c]);
+                            }
+                    } else {
                     Real dx[RX], dx2[RX], dy[RY], dy2[RY];
 #pragma unroll
                     for (int c = 0; c < RX; ++c) { dx[c] = sub_rn(ox[c], l.x); dx2[c] = mul_rn(dx[c], dx[c]); }
@@ -279,6 +332,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
                             sx[r][c] = fma_rn(dx[c], inv, sx[r][c]);
                             sy[r][c] = fma_rn(dy[r], inv, sy[r][c]);
                         }
+                    } // regular grid
                 }
             }
             // flush the group's partial sums into the fp64 accumulators
@@ -295,7 +349,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
         buf ^= 1;
     }
 
-    finish_tile<RX, RY, CAPTURE>(p, ti, tj, t, lane, warp, Sx, Sy, cta_count);
+    finish_tile<RX, RY, CAPTURE, kWarps, RANDOM>(p, ti, tj, t, lane, warp, Sx, Sy, cta_count);
 }
 
 // ---------------------------------------------------------------------------------------

@@ -54,6 +54,9 @@ class MagnificationMap:
         else:
             _b.ml_set_lens_masses(self._ctx, xy, mass)
 
+    def set_ray_mode(self, mode, seed=0):
+        _b.ml_set_ray_mode(self._ctx, mode, seed)
+
     def set_precision(self, mode):
         _b.ml_set_precision(self._ctx, mode)
 

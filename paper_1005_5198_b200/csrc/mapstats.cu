@@ -70,8 +70,12 @@ __global__ void __launch_bounds__(kPassThreads, 1) pass_kernel(const unsigned in
     p.max_a = p.max_b = 0u;
     const bool vec = ((reinterpret_cast<uintptr_t>(a) & 15) == 0) && (!TWO || (reinterpret_cast<uintptr_t>(b) & 15) == 0);
     const long long stride = (long long)gridDim.x * kPassThreads * 4;
-    for (long long i = ((long long)blockIdx.x * kPassThreads + threadIdx.x) * 4; i < n; i += stride) {
-        unsigned int ca[4] = {0, 0, 0, 0}, cb[4] = {0, 0, 0, 0};
+    unsigned int n_valid = 0, n_empty_a = 0, n_empty_b = 0; // per thread: < 2^31 / (gridDim.x * 1024) pixels each
+
+    auto load4 = [&](long long i, unsigned int (&ca)[4], unsigned int (&cb)[4]) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { ca[q] = 0u; cb[q] = 0u; }
+        if (i >= n) return;
         if (vec && i + 3 < n) {
             const uint4 va = *reinterpret_cast<const uint4 *>(a + i);
             ca[0] = va.x; ca[1] = va.y; ca[2] = va.z; ca[3] = va.w;
@@ -87,6 +91,37 @@ __global__ void __launch_bounds__(kPassThreads, 1) pass_kernel(const unsigned in
                     if (TWO) cb[q] = b[i + q];
                 }
         }
+    };
+    auto process4 = [&](long long i, const unsigned int (&ca)[4], const unsigned int (&cb)[4]) {
+        if (i >= n) return;
+        const unsigned int big = ca[0] | ca[1] | ca[2] | ca[3] | cb[0] | cb[1] | cb[2] | cb[3];
+        if (i + 3 < n && big < kLut) {
+            // common case: four pixels, every count inside the log table and the shared-memory bins: no range checks
+            unsigned int s_a = 0, s_b = 0;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                atomicAdd(&sh_a[ca[q]], 1u);
+                if (TWO) atomicAdd(&sh_b[cb[q]], 1u);
+                if (STATS) {
+                    s_a += ca[q];
+                    p.max_a = max(p.max_a, ca[q]);
+                    n_empty_a += (ca[q] == 0);
+                    if (TWO) {
+                        s_b += cb[q];
+                        p.max_b = max(p.max_b, cb[q]);
+                        n_empty_b += (cb[q] == 0);
+                        const bool valid = (ca[q] != 0) & (cb[q] != 0);
+                        // dm_a - dm_b = -2.5 (log10 N_a - log10 N_b - log10(n_rays_a / n_rays_b))   (eq. 10)
+                        const double d = -2.5 * ((sh_log[ca[q]] - sh_log[cb[q]]) - log_rays);
+                        p.ssq += valid ? d * d : 0.0;
+                        n_valid += valid;
+                    }
+                }
+            }
+            p.sum_a += s_a;
+            p.sum_b += s_b;
+            return;
+        }
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             if (i + q >= n) break;
@@ -95,23 +130,31 @@ __global__ void __launch_bounds__(kPassThreads, 1) pass_kernel(const unsigned in
             if (STATS) {
                 p.sum_a += ca[q];
                 p.max_a = max(p.max_a, ca[q]);
-                p.n_empty_a += (ca[q] == 0);
+                n_empty_a += (ca[q] == 0);
                 if (TWO) {
                     p.sum_b += cb[q];
                     p.max_b = max(p.max_b, cb[q]);
-                    p.n_empty_b += (cb[q] == 0);
+                    n_empty_b += (cb[q] == 0);
                     if (ca[q] > 0 && cb[q] > 0) {
-                        // dm_a - dm_b = -2.5 (log10 N_a - log10 N_b - log10(n_rays_a / n_rays_b))   (eq. 10)
                         const double la = ca[q] < kLut ? sh_log[ca[q]] : log10((double)ca[q]);
                         const double lb = cb[q] < kLut ? sh_log[cb[q]] : log10((double)cb[q]);
                         const double d = -2.5 * ((la - lb) - log_rays);
                         p.ssq += d * d;
-                        p.n_valid += 1;
+                        n_valid += 1;
                     }
                 }
             }
         }
+    };
+    // two quads in flight per thread: the loads of the second are issued before the first is processed
+    for (long long i = ((long long)blockIdx.x * kPassThreads + threadIdx.x) * 4; i < n; i += 2 * stride) {
+        unsigned int ca0[4], cb0[4], ca1[4], cb1[4];
+        load4(i, ca0, cb0);
+        load4(i + stride, ca1, cb1);
+        process4(i, ca0, cb0);
+        process4(i + stride, ca1, cb1);
     }
+    p.n_valid = n_valid; p.n_empty_a = n_empty_a; p.n_empty_b = n_empty_b;
     __syncthreads();
     for (unsigned int k = threadIdx.x; k < kShBins; k += kPassThreads) {
         const unsigned int va = sh_a[k];

@@ -135,6 +135,8 @@ def run_reference(args):
         return 0
     p = pick(args.workload)
     per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    if args.ref_seconds_per_step is not None:
+        per_step = args.ref_seconds_per_step
     for _ in range(args.warmup):
         oracle_rate(p, per_step)
     inter, secs, last = 0, 0.0, None
@@ -436,6 +438,8 @@ def main():
     ap.add_argument("--n-lenses", type=int, default=0, help="override the lens count (large-N* row); 0 = eq. 5")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-seconds-per-step", type=float, default=None,
+                    help="--impl reference: oracle seconds per step (default: 120 s spread over steps + warmup, 1-20 s each)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: note: --warmup < 3 breaks the timing rules", file=sys.stderr)

@@ -63,7 +63,7 @@ enum {
                                      lenses flushed into fp64 accumulators, fp64 epilogue    */
     ML_PREC_FP32_COMPENSATED = 1, /* as above, Newton-refined reciprocal and a flush every
                                      8 lenses                                                */
-    ML_PREC_FP64 = 2              /* everything in fp64 (true division)                      */
+    ML_PREC_FP64 = 2              /* everything in fp64 (reciprocal refined to an ulp)       */
 };
 
 /* Where the rays start.  REGULAR: the cell-centred regular grid of the configs

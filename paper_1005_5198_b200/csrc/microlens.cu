@@ -62,7 +62,7 @@ struct Mode {
 constexpr int RXF = 4, RYF = 4, KFF = 64;  // FP32_TILED (shoot_kernel_pipe) and FP32_COMPENSATED
 constexpr int WARPS_T = 4, SHARED_T = 4, MINB_T = 3; // FP32_TILED: 128-thread CTAs, 3 per SM, all rows share
 constexpr int KFC = 8;                     // FP32_COMPENSATED
-constexpr int RXD = 2, RYD = 2, KFD = 64;  // FP64
+constexpr int RXD = 4, RYD = 2, KFD = 64;  // FP64
 
 constexpr int RXR = 4, RYR = 2;            // FP32 modes with random rays: every ray carries its own offsets
 

@@ -71,8 +71,9 @@ template <typename Real, bool NEWTON> __device__ __forceinline__ Real pad_coordi
 template <> __device__ __forceinline__ float pad_coordinate<float, false>() { return 1e30f; }
 // with the Newton step inf * 0 would give NaN: stay finite (term ~ 5e-19, below every rounding)
 template <> __device__ __forceinline__ float pad_coordinate<float, true>() { return 1e18f; }
-template <> __device__ __forceinline__ double pad_coordinate<double, false>() { return 1e200; }
-template <> __device__ __forceinline__ double pad_coordinate<double, true>() { return 1e200; }
+// fp64: r^2 = 2e200 stays finite (the Newton-refined reciprocal below would turn inf * 0 into NaN); term ~ 5e-101
+template <> __device__ __forceinline__ double pad_coordinate<double, false>() { return 1e100; }
+template <> __device__ __forceinline__ double pad_coordinate<double, true>() { return 1e100; }
 
 __device__ __forceinline__ float rcp_approx(float a)
 {
@@ -90,7 +91,18 @@ template <bool NEWTON> __device__ __forceinline__ float recip(float a)
     }
     return r;
 }
-template <bool NEWTON> __device__ __forceinline__ double recip(double a) { return 1.0 / a; }
+// fp64 reciprocal: MUFU.RCP64H seed (rcp.approx.ftz.f64, ~20 bits) + two Newton-Raphson steps (4 DFMA): within an
+// ulp of 1/a for the normal, finite r^2 that occur, without the IEEE division's slow-path fix-up (about half its
+// instructions).  a = 0 (ray on a lens) gives inf -> NaN -> the ray is dropped, as in the oracle (R12).
+template <bool NEWTON> __device__ __forceinline__ double recip(double a)
+{
+    double x;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(a));
+    double e = __fma_rn(-a, x, 1.0);
+    x = __fma_rn(x, e, x);
+    e = __fma_rn(-a, x, 1.0);
+    return __fma_rn(x, e, x);
+}
 
 __device__ __forceinline__ float sub_rn(float a, float b) { return __fsub_rn(a, b); }
 __device__ __forceinline__ double sub_rn(double a, double b) { return __dsub_rn(a, b); }

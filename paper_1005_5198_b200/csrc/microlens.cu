@@ -61,7 +61,8 @@ struct Mode {
 };
 constexpr int RXF = 4, RYF = 4, KFF = 64;  // FP32_TILED (shoot_kernel_pipe) and FP32_COMPENSATED
 constexpr int WARPS_T = 4, SHARED_T = 4, MINB_T = 3; // FP32_TILED: 128-thread CTAs, 3 per SM, all rows share
-constexpr int KFC = 8;                     // FP32_COMPENSATED
+constexpr int KFC = 8;                     // FP32_COMPENSATED, generic kernel (random rays)
+constexpr int KFCP = 16;                   // FP32_COMPENSATED, regular grid: the pipe kernel with a Newton step
 constexpr int RXD = 4, RYD = 2, KFD = 64;  // FP64
 
 constexpr int RXR = 4, RYR = 2;            // FP32 modes with random rays: every ray carries its own offsets
@@ -70,8 +71,7 @@ Mode mode_of(int precision, int ray_mode)
 {
     if (precision == ML_PREC_FP64) return {32 * RXD, kWarps * RYD};
     if (ray_mode == ML_RAYS_RANDOM) return {32 * RXR, kWarps * RYR};
-    if (precision == ML_PREC_FP32_TILED) return {32 * RXF, WARPS_T * RYF};
-    return {32 * RXF, kWarps * RYF};
+    return {32 * RXF, WARPS_T * RYF};
 }
 
 Mode mode_of(const ml_ctx *c) { return mode_of(c->precision, c->ray_mode); }
@@ -83,7 +83,7 @@ template <bool CAPTURE, bool MASS> cudaError_t launch_m(int precision, unsigned 
         shoot_kernel<double, RXD, RYD, KFD, false, CAPTURE, MASS><<<g, kThreads, 0, s>>>(p);
         break;
     case ML_PREC_FP32_COMPENSATED:
-        shoot_kernel<float, RXF, RYF, KFC, true, CAPTURE, MASS><<<g, kThreads, 0, s>>>(p);
+        shoot_kernel_pipe<SHARED_T, KFCP, WARPS_T, MINB_T, true, CAPTURE, MASS, true><<<g, WARPS_T * 32, 0, s>>>(p);
         break;
     default:
         shoot_kernel_pipe<SHARED_T, KFF, WARPS_T, MINB_T, true, CAPTURE, MASS><<<g, WARPS_T * 32, 0, s>>>(p);

@@ -398,7 +398,7 @@ template <int RY> struct PipeRegs {
     float2 R[RY];
 };
 
-template <int SHARED, int KF, int WARPS, int MINB, bool SCALAR_DY, bool CAPTURE, bool MASS = false>
+template <int SHARED, int KF, int WARPS, int MINB, bool SCALAR_DY, bool CAPTURE, bool MASS = false, bool NEWTON = false>
 __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const ShootParams p)
 {
     constexpr int RX = 4, RY = 4;
@@ -425,7 +425,10 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
         tj = p.tile_j0 + t / p.tiles_x;
     }
     if (threadIdx.x < 3) cta_count[threadIdx.x] = 0;
-    if (threadIdx.x < 4) lens_s[threadIdx.x >> 1][kChunk + (threadIdx.x & 1)] = make_float4(-1e15f, -1e15f, -1e15f, -1e15f);
+    // NEWTON: the padding lens must keep r2A * r2B finite (inf * 0 in the refinement would be NaN): 1e9 -> product 4e36,
+    // its terms are 5e-10 R_E (at most two padding lenses per launch are ever evaluated: below every tolerance)
+    const float padc = NEWTON ? -1e9f : -1e15f;
+    if (threadIdx.x < 4) lens_s[threadIdx.x >> 1][kChunk + (threadIdx.x & 1)] = make_float4(padc, padc, padc, padc);
     if (MASS && threadIdx.x < 4) mass_s[threadIdx.x >> 1][(MASS ? kChunk : 0) + (MASS ? (threadIdx.x & 1) : 0)] = 0.f;
 
     const double cx = ((double)(ti * TW) + 0.5 * (TW - 1) - p.half1) * p.delta;
@@ -464,7 +467,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
 #pragma unroll
         for (int q = 0; q < PER_THREAD; ++q) {
             const int k = base + q * THREADS + threadIdx.x;
-            float nx = -1e15f, ny = -1e15f, m = 0.f;
+            float nx = padc, ny = padc, m = 0.f;
             if (k < p.n_lens) {
                 nx = -(float)(pre[q].x - cx);
                 ny = -(float)(pre[q].y - cy);
@@ -512,7 +515,13 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
         for (int r = 0; r < RY; ++r) {
             float2 iA, iB;
             if (r < SHARED) {
-                const float2 R = MASS ? __fmul2_rn(s.R[r], make_float2(s.m, s.m)) : s.R[r]; // m_i / (r2A r2B)
+                float2 R = s.R[r];
+                if (NEWTON) { // one Newton-Raphson step on the shared reciprocal: R <- R + R (1 - P R), P = r2A r2B
+                    const float2 P = __fmul2_rn(s.r2A[r], s.r2B[r]);
+                    const float2 e = __ffma2_rn(make_float2(-P.x, -P.y), R, make_float2(1.f, 1.f));
+                    R = __ffma2_rn(R, e, R);
+                }
+                if (MASS) R = __fmul2_rn(R, make_float2(s.m, s.m)); // m_i / (r2A r2B)
                 iA = __fmul2_rn(R, s.r2B[r]);
                 iB = __fmul2_rn(R, s.r2A[r]);
             } else {

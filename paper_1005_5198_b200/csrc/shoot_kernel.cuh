@@ -93,7 +93,7 @@ template <bool NEWTON> __device__ __forceinline__ float recip(float a)
 }
 // fp64 reciprocal: MUFU.RCP64H seed (rcp.approx.ftz.f64, ~20 bits) + two Newton-Raphson steps (4 DFMA): within an
 // ulp of 1/a for the normal, finite r^2 that occur, without the IEEE division's slow-path fix-up (about half its
-// instructions).  a = 0 (ray on a lens) gives inf -> NaN -> the ray is dropped, as in the oracle (R12).
+// instructions).  a = 0 (ray on a lens) gives inf -> NaN -> the ray is dropped (reading R12).
 template <bool NEWTON> __device__ __forceinline__ double recip(double a)
 {
     double x;

@@ -5,7 +5,7 @@
 // Delta m = -2.5 log10(mu) (eq. 10), mu = N/N_rays (eq. 3).
 //
 // Counts are integers, so the K-S distance needs no sort: one fused pass over both maps gathers
-// the RMS sums, the map statistics and the two count histograms (warp-aggregated RED into L2);
+// the RMS sums, the map statistics and the two count histograms (per-CTA shared-memory bins, flushed once);
 // prefix sums of the histograms are the two empirical distributions, and
 //   D = max over sample points x of |F_a(x) - F_b(x)|
 // is evaluated at the sample points of both maps (x = c/n_rays_a and x = c/n_rays_b, compared in

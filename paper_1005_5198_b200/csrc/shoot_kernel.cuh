@@ -141,7 +141,7 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
     constexpr int TW = 32 * RX;
     constexpr int TH = WARPS * RY;
     // ---- a4 + a5: macro terms, pixel, binning
-    unsigned int n_shot = 0, n_in = 0, n_drop = 0; // warp-uniform
+    unsigned int n_shot = 0, n_in = 0, n_drop = 0; // per thread; reduced over the warp once, after the loop
     const unsigned int full = 0xffffffffu;
 #pragma unroll
     for (int r = 0; r < RY; ++r) {
@@ -179,19 +179,21 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
                 const int prev = __shfl_up_sync(full, pix, 1);
                 const bool head = (lane == 0) || (pix != prev);
                 const unsigned int heads = __ballot_sync(full, head);
-                const unsigned int inmask = __ballot_sync(full, pix >= 0);
                 if (head && pix >= 0) {
                     const unsigned int above = heads & ~((2u << lane) - 1u);
                     const int next = above ? (__ffs(above) - 1) : 32;
                     atomicAdd(&p.map[pix], (unsigned int)(next - lane));
                 }
-                n_in += __popc(inmask);
-                n_shot += __popc(__ballot_sync(full, valid));
-                n_drop += __popc(__ballot_sync(full, valid && !finite));
+                n_in += (pix >= 0);
+                n_shot += valid;
+                n_drop += (valid && !finite);
             }
         }
     }
     if (!CAPTURE) {
+        n_shot = __reduce_add_sync(full, n_shot); // REDUX.SUM: one instruction per counter instead of a vote per ray
+        n_in = __reduce_add_sync(full, n_in);
+        n_drop = __reduce_add_sync(full, n_drop);
         if (lane == 0) {
             atomicAdd(&cta_count[0], n_shot);
             atomicAdd(&cta_count[1], n_in);

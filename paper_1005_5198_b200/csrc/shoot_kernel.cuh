@@ -143,15 +143,29 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
     // ---- a4 + a5: macro terms, pixel, binning
     unsigned int n_shot = 0, n_in = 0, n_drop = 0; // per thread; reduced over the warp once, after the loop
     const unsigned int full = 0xffffffffu;
+    // per-column / per-row quantities once per thread: image-plane coordinate and "inside the requested region" bits
+    double x1c[RX];
+    unsigned int colmask = 0u, rowmask = 0u;
+#pragma unroll
+    for (int c = 0; c < RX; ++c) {
+        const long long i = ti * TW + lane * RX + c;
+        x1c[c] = ((double)i - p.half1) * p.delta;
+        colmask |= ((i >= p.i0) && (i < p.i1)) ? (1u << c) : 0u;
+    }
+#pragma unroll
+    for (int r = 0; r < RY; ++r) {
+        const long long j = tj * TH + warp * RY + r;
+        rowmask |= ((j >= p.j0) && (j < p.j1)) ? (1u << r) : 0u;
+    }
+    const unsigned int n_pix_u = (unsigned int)p.n_pix;
 #pragma unroll
     for (int r = 0; r < RY; ++r) {
         const long long j = tj * TH + warp * RY + r;
         double x2 = ((double)j - p.half2) * p.delta;
-        const bool jvalid = (j >= p.j0) && (j < p.j1);
 #pragma unroll
         for (int c = 0; c < RX; ++c) {
             const long long i = ti * TW + lane * RX + c;
-            double x1 = ((double)i - p.half1) * p.delta;
+            double x1 = x1c[c];
             if (RANDOM) { // the ray's own position in its cell (same draw as in the prologue)
                 double u1, u2;
                 ray_uniforms((unsigned long long)j * (unsigned long long)p.n1 + (unsigned long long)i, p.ray_seed, u1, u2);
@@ -168,13 +182,13 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
                 o.y = finite ? y2 : qnan;
                 p.capture[(size_t)t * (TW * TH) + (size_t)(warp * RY + r) * TW + lane * RX + c] = o;
             } else {
-                const bool valid = jvalid && (i >= p.i0) && (i < p.i1);
+                const bool valid = ((colmask >> c) & (rowmask >> r) & 1u) != 0u;
                 const double u1 = (y1 + p.halfL) * p.inv_pixel;
                 const double u2 = (y2 + p.halfL) * p.inv_pixel;
-                const double np = (double)p.n_pix;
-                const bool inside = (u1 >= 0.0) && (u1 < np) && (u2 >= 0.0) && (u2 < np);
-                int pix = -1;
-                if (valid && finite && inside) pix = (int)u2 * p.n_pix + (int)u1;
+                // floor to int (saturating): 0 <= u < n_pix  <=>  (unsigned)floor(u) < n_pix for every finite u
+                const int pi = __double2int_rd(u1), pj = __double2int_rd(u2);
+                const bool inside = ((unsigned int)pi < n_pix_u) && ((unsigned int)pj < n_pix_u);
+                const int pix = (valid && finite && inside) ? pj * p.n_pix + pi : -1;
                 // run-length aggregation along the lanes of the warp
                 const int prev = __shfl_up_sync(full, pix, 1);
                 const bool head = (lane == 0) || (pix != prev);

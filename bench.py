@@ -8,12 +8,18 @@ generation, deflection sum, macro terms, binning; map zeroing included) over the
 grid of the workload: one ml_shoot (N = 1) or one row band per rank plus the map all-reduce
 (N > 1, strong scaling).  Prints ONE JSON line (rank 0).  DESIGN.md "Measurement" explains
 every field.
+
+N > 1: one process per GPU over NCCL.  Started under torchrun the ranks come from the
+environment; started as plain `python bench.py --gpus N` the script launches the N ranks
+itself (torch.distributed.run on 127.0.0.1).  Fewer than N visible GPUs is an error -- the
+script never runs fewer GPUs than it prints.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
 import subprocess
 import sys
 import tempfile
@@ -177,55 +183,169 @@ def config_dict(p, info, args):
 
 # ------------------------------------------------------------------ the CUDA arm
 PRECISIONS = {"fp32_tiled": 0, "fp32_compensated": 1, "fp64": 2}
+# per_config block of the default line: (workload, timed steps, full warm-up steps); configs without a full warm-up step
+# are warmed by three shoots of 1/32 of their ray rows (the device is already warm from the C2 region before them)
+PER_CONFIG_PLAN = (("C1", 50, 5), ("C5", 2, 0), ("C3", 1, 0), ("C4", 1, 0))
+
+
+def fp32_peak_tflops(info):
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    max_mhz = float(peaks.get("sm_max_mhz") or (info["sm_clock_khz"] / 1e3))
+    return int(info["sm_count"]) * FP32_LANES_PER_SM * 2 * max_mhz * 1e6 / 1e12, max_mhz
+
+
+class ShootRig:
+    """One workload set up the way a user of the library would: context, lenses, a torch-owned device map, a torch
+    stream attached to the context, pinned host buffers for the end-to-end leg."""
+
+    def __init__(self, ml, torch, p, args, local, rank=0, world=1, flush=None):
+        from paper_1005_5198_b200.sharding import row_band
+        self.torch, self.p, self.world = torch, p, world
+        self.dev = torch.device("cuda", local)
+        self.m = ml.MagnificationMap(*problem_args(p), device=local, precision=PRECISIONS[args.precision])
+        info = self.m.info
+        n_field = args.n_lenses if args.n_lenses > 0 else info["n_star_expected"]
+        self.xy = lens_disk(n_field, info["r_star"], p.seed)
+        self.mass = lens_masses(n_field, p.seed) if args.masses else None
+        self.m.set_lenses(self.xy, self.mass)
+        if args.random_rays:
+            self.m.set_ray_mode(ml.ML_RAYS_RANDOM, 20100527)
+        self.info = info = self.m.info
+        self.n1, self.n2, self.n_lens = int(info["n1"]), int(info["n2"]), int(info["n_lenses"])
+        self.j0, self.j1 = row_band(self.n2, rank, world, int(info["tile_h"]))
+        self.stream = torch.cuda.Stream(device=self.dev)
+        self.counts = torch.zeros((p.n_pix, p.n_pix), dtype=torch.int32, device=self.dev)  # torch owns the map memory
+        self.m.use_device_map(self.counts.data_ptr())
+        self.m.attach_stream(self.stream.cuda_stream)
+        self.flush = flush if flush is not None else torch.empty(256 << 20, dtype=torch.uint8, device=self.dev)
+        self.host_xy = torch.from_numpy(self.xy).pin_memory()
+        self.host_map = torch.empty((p.n_pix, p.n_pix), dtype=torch.int32).pin_memory()
+        self.host_map_np = self.host_map.numpy().view(np.uint32)
+
+    def flush_l2(self):
+        with self.torch.cuda.stream(self.stream):
+            self.flush.fill_(1)                  # 256 MiB write: evicts the 126 MB L2
+
+    def step(self, rows=None):
+        """flush L2, zero the map, shoot this rank's band, (N > 1) all-reduce the maps; returns ml_stats."""
+        from paper_1005_5198_b200.sharding import allreduce_map
+        j0, j1 = rows if rows is not None else (self.j0, self.j1)
+        self.flush_l2()
+        self.m.shoot_region(0, self.n1, j0, j1)  # zero map + fused kernel (synchronises the stream)
+        st = self.m.stats
+        if self.world > 1:
+            with self.torch.cuda.stream(self.stream):
+                allreduce_map(self.counts)
+        return st
+
+    def e2e_step(self):
+        """The same through the C ABI with HOST buffers: lenses host -> device, shoot, map device -> host."""
+        from paper_1005_5198_b200.sharding import allreduce_map
+        self.m.set_lenses(self.host_xy.numpy(), self.mass)   # H2D (ml_set_lenses / ml_set_lens_masses)
+        self.m.shoot_region(0, self.n1, self.j0, self.j1)
+        st = self.m.stats
+        if self.world > 1:
+            with self.torch.cuda.stream(self.stream):
+                allreduce_map(self.counts)
+        self.m.counts(out=self.host_map_np)                  # D2H (ml_get_map)
+        return st
+
+    def e2e_bytes(self):
+        h2d = int(self.xy.nbytes) + (int(self.mass.nbytes) if self.mass is not None else 0)
+        return h2d, int(self.host_map_np.nbytes + 24)
+
+    def close(self):
+        self.m.close()
+
+
+def per_config_entry(ml, torch, name, steps, full_warmup, args, local, flush):
+    """One entry of the default line's per_config block (single GPU).  Every timed step is an END-TO-END step (host
+    lenses -> ml_set_lenses -> ml_shoot -> ml_get_map -> host map, L2 flushed before it, outside the clock): `e2e` is
+    its wall clock, `kernel_ms` the library's CUDA events around the kernel launch of the same step, `value` the
+    device-timed rate of the whole step without the copies (memset + kernel, events on the launching stream)."""
+    p = pick(name)
+    rig = ShootRig(ml, torch, p, args, local, flush=flush)
+    dev, n_lens, rays = rig.dev, rig.n_lens, rig.n1 * rig.n2
+    for _ in range(full_warmup):
+        rig.step()
+    if not full_warmup:
+        band = max(int(rig.info["tile_h"]), rig.n2 // 32)
+        for k in range(3):
+            rig.step(rows=(k * band, (k + 1) * band))
+    sampler = ClockSampler(local)
+    short = rays * n_lens < 1e11          # ms-long steps: a polling nvidia-smi triples their host latency
+    if short:
+        sampler.start()
+        t_end = time.perf_counter() + 1.2
+        while time.perf_counter() < t_end:
+            rig.step()
+        clocks = sampler.stop()
+        clocks["when"] = "1.2 s of the same steps immediately before the timed region"
+    else:
+        sampler.start()
+    kernel_ms, dev_ms, wall = 0.0, 0.0, 0.0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(steps):
+        rig.flush_l2()
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        st = rig.e2e_step()
+        wall += time.perf_counter() - t0
+        assert int(st["rays_shot"]) == rays
+        kernel_ms += st["kernel_ms"]
+        rig.flush_l2()                    # the device-timed form of the same step: memset + kernel, no copies
+        e0.record(rig.stream)
+        rig.m.shoot_region(0, rig.n1, 0, rig.n2)
+        e1.record(rig.stream)
+        torch.cuda.synchronize(dev)
+        dev_ms += e0.elapsed_time(e1)
+        kernel_ms += rig.m.stats["kernel_ms"]
+    if not short:
+        clocks = sampler.stop()
+    peak, _ = fp32_peak_tflops(rig.info)
+    inter = float(rays) * n_lens
+    h2d, d2h = rig.e2e_bytes()
+    k_ms = kernel_ms / (2 * steps)
+    out = {"workload": config_dict(p, rig.info, args)["workload"], "n_lenses": n_lens, "rays": rays, "steps": steps,
+           "kernel_ms": k_ms, "ms_per_step": dev_ms / steps, "value": inter * steps / (dev_ms * 1e-3), "unit": UNIT,
+           "frac": N_FLOP * inter / (k_ms * 1e-3) / 1e12 / peak,
+           "step_frac": N_FLOP * inter * steps / (dev_ms * 1e-3) / 1e12 / peak,
+           "e2e": {"value": inter * steps / wall, "unit": UNIT, "ms_per_step": 1e3 * wall / steps,
+                   "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+           "clocks": clocks,
+           "note": "each config is shot 2 x steps times: once end to end (host buffers, wall clock) and once device-timed"}
+    rig.close()
+    return out
 
 
 def run_ours(args):
     import torch
     import torch.distributed as dist
     import paper_1005_5198_b200 as ml
-    from paper_1005_5198_b200.sharding import allreduce_map, row_band
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; --impl reference times the oracle)")
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d: launch with --nproc-per-node equal to --gpus"
+                         % (args.gpus, world))
+    if local >= torch.cuda.device_count():
+        raise SystemExit("bench.py: rank %d needs cuda:%d but only %d device(s) are visible"
+                         % (rank, local, torch.cuda.device_count()))
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-    assert world == args.gpus or world == 1, "launch with torchrun --nproc-per-node == --gpus"
 
     p = pick(args.workload)
-    m = ml.MagnificationMap(*problem_args(p), device=local, precision=PRECISIONS[args.precision])
-    info = m.info
-    n_field = args.n_lenses if args.n_lenses > 0 else info["n_star_expected"]
-    xy = lens_disk(n_field, info["r_star"], p.seed)
-    mass = lens_masses(n_field, p.seed) if args.masses else None
-    m.set_lenses(xy, mass)
-    if args.random_rays:
-        m.set_ray_mode(ml.ML_RAYS_RANDOM, 20100527)
-    info = m.info
-    n1, n2, n_lens = int(info["n1"]), int(info["n2"]), int(info["n_lenses"])
-    j0, j1 = row_band(n2, rank, world, int(info["tile_h"]))
-
-    stream = torch.cuda.Stream(device=dev)
-    counts = torch.zeros((p.n_pix, p.n_pix), dtype=torch.int32, device=dev)  # torch owns the map memory
-    m.use_device_map(counts.data_ptr())
-    m.attach_stream(stream.cuda_stream)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    host_xy = torch.from_numpy(xy).pin_memory()
-    host_map = torch.empty((p.n_pix, p.n_pix), dtype=torch.int32).pin_memory()
-    host_map_np = host_map.numpy().view(np.uint32)
-
-    def step():
-        with torch.cuda.stream(stream):
-            flush.fill_(1)                       # evict L2 between steps
-            m.shoot_region(0, n1, j0, j1)        # zero map + fused kernel (synchronises `stream`)
-            st = m.stats
-            if world > 1:
-                allreduce_map(counts)
-        return st
+    rig = ShootRig(ml, torch, p, args, local, rank, world)
+    info, n1, n2, n_lens, stream = rig.info, rig.n1, rig.n2, rig.n_lens, rig.stream
 
     def barrier():
         if world > 1:
@@ -233,7 +353,7 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
 
     for _ in range(args.warmup):
-        step()
+        rig.step()
     sampler = ClockSampler(local)
     barrier()
     if rank == 0:
@@ -243,7 +363,7 @@ def run_ours(args):
     barrier()
     e0.record(stream)
     for _ in range(args.steps):
-        st = step()
+        st = rig.step()
         kernel_ms += st["kernel_ms"]
         launches += int(st["kernel_launches"])
         rays += int(st["rays_shot"])
@@ -266,48 +386,50 @@ def run_ours(args):
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
-        m.set_lenses(host_xy.numpy(), mass)      # H2D: lens positions (host buffer -> ml_set_lenses)
-        m.shoot_region(0, n1, j0, j1)
-        if world > 1:
-            with torch.cuda.stream(stream):
-                allreduce_map(counts)
-        m.counts(out=host_map_np)                # D2H: the map (ml_get_map -> host buffer)
+        rig.e2e_step()
     barrier()
     e2e_s = time.perf_counter() - t0
     e2e_t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
     if world > 1:
         dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
     e2e_value = n1 * n2 * n_lens * e2e_steps / float(e2e_t[0])
-    m.close()
+    h2d, d2h = rig.e2e_bytes()
+    flush = rig.flush
+    rig.close()
     if world > 1:
         dist.destroy_process_group()
     if rank != 0:
         return 0
 
+    peak_tflops, max_mhz = fp32_peak_tflops(info)
     sm_count = int(info["sm_count"])
-    peaks = {}
-    try:
-        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-    except Exception:
-        pass
-    max_mhz = float(peaks.get("sm_max_mhz") or (info["sm_clock_khz"] / 1e3))
-    peak_tflops = sm_count * FP32_LANES_PER_SM * 2 * max_mhz * 1e6 / 1e12
     kernel_s_per_launch = kernel_ms_max * 1e-3 / max(1, launches_all // max(world, 1))
     inter_per_launch = (rays_all // world) * n_lens / max(1, launches_all // max(world, 1))
     achieved = N_FLOP * inter_per_launch / kernel_s_per_launch / 1e12
+    # ncu DRAM bytes exist only for the exact kernel that was captured: the BASELINE workload, unit masses, regular grid
+    plain = world == 1 and not (args.masses or args.random_rays or args.n_lenses > 0)
+    traffic, traffic_src = NCU_DRAM_BYTES_PER_LAUNCH.get((p.name, args.precision), (None, None)) if plain else (None, None)
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops,
-                "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get((p.name, args.precision), (None, None))[0] if world == 1 else None,
+                "frac": achieved / peak_tflops, "traffic": traffic,
                 "traffic_unit": "bytes of DRAM traffic per launch (ncu --set full; %s); algorithmic HBM bytes per "
                                 "launch = n_pix^2*4 map + 16*N* lenses = %d"
-                                % (NCU_DRAM_BYTES_PER_LAUNCH.get((p.name, args.precision), (None, "no capture"))[1],
-                                   p.n_pix * p.n_pix * 4 + 16 * n_lens),
+                                % (traffic_src or "no capture of this kernel instantiation", p.n_pix * p.n_pix * 4 + 16 * n_lens),
                 "note": "nominal %g flop/interaction (PAPER.md:66); peak = %d SMs x 128 FP32 lanes x 2 x %.0f MHz "
                         "(MEASURED_PEAKS.json sm_max_mhz); kernel time = CUDA events on the launching stream"
                         % (N_FLOP, sm_count, max_mhz),
                 "kernel_ms_per_launch": 1e3 * kernel_s_per_launch}
     if clocks and clocks.get("sm_mhz"):
         roofline["frac_at_sampled_clock"] = achieved / (peak_tflops * clocks["sm_mhz"] / max_mhz)
+    per_config = None
+    if plain and args.workload == "C2" and args.precision == "fp32_tiled" and not args.no_per_config:
+        per_config = [{"workload": config_dict(p, info, args)["workload"], "n_lenses": n_lens, "rays": n1 * n2,
+                       "steps": args.steps, "kernel_ms": 1e3 * kernel_s_per_launch, "ms_per_step": ms / args.steps,
+                       "value": value, "unit": UNIT, "frac": achieved / peak_tflops,
+                       "step_frac": N_FLOP * value / 1e12 / peak_tflops,
+                       "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+                       "clocks": clocks, "note": "the line's own timed region"}]
+        for name, steps, full_warmup in PER_CONFIG_PLAN:
+            per_config.append(per_config_entry(ml, torch, name, steps, full_warmup, args, local, flush))
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         cpu = oracle_rate(p, args.cpu_seconds)
@@ -319,11 +441,30 @@ def run_ours(args):
             "rays_per_s": rays_all / (ms * 1e-3), "map_wall_ms": ms / args.steps,
             "nominal_tflops": N_FLOP * value / 1e12, "frac_fp32_peak": N_FLOP * value / 1e12 / (peak_tflops * args.gpus),
             "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(xy.nbytes),
-                    "d2h_bytes_per_step": int(host_map_np.nbytes + 24), "steps": e2e_steps},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "steps": e2e_steps},
             "gpu_launches": launches_all}
+    if per_config is not None:
+        line["per_config"] = per_config
     print(json.dumps(line))
     return 0
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` with N > 1 and no torchrun around it: start the N ranks here (one process per GPU,
+    NCCL over 127.0.0.1) and pass their exit code on.  Refuses to run with fewer than N devices."""
+    import torch
+    have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    if have < args.gpus:
+        print("bench.py: --gpus %d requested but %d CUDA device(s) are visible; refusing to run fewer GPUs than reported"
+              % (args.gpus, have), file=sys.stderr)
+        return 2
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 # ------------------------------------------------------------------ the map-comparison row (SURVEY.md 8(f) item 2)
@@ -438,14 +579,22 @@ def main():
     ap.add_argument("--n-lenses", type=int, default=0, help="override the lens count (large-N* row); 0 = eq. 5")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true",
+                    help="skip the per_config block (C1, C5, C3, C4 after the C2 timed region) of the default line")
     ap.add_argument("--ref-seconds-per-step", type=float, default=None,
                     help="--impl reference: oracle seconds per step (default: 120 s spread over steps + warmup, 1-20 s each)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         print("bench.py: note: --warmup < 3 breaks the timing rules", file=sys.stderr)
-    if args.row == "mapstats" and args.impl == "ours":
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.row == "mapstats":
         return run_mapstats(args)
-    return run_reference(args) if args.impl == "reference" else run_ours(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_ranks(args)
+    return run_ours(args)
 
 
 if __name__ == "__main__":

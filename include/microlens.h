@@ -107,6 +107,8 @@ typedef struct {
     uint64_t kernel_launches; /* launches of the shoot kernel since the map was last zeroed   */
     double kernel_ms;      /* device time of those launches, CUDA events on the ctx stream    */
     double total_ms;       /* host wall time of the last ml_shoot / ml_shoot_region call      */
+    uint64_t capture_ctas; /* CTAs of the last launch that split its lens loop (tiles x lens ranges:
+                              ml_probe / ml_capture_region / a small ml_shoot_region at N* >= 8192); else 0 */
 } ml_stats;
 
 /* Create a context for one map.  Arguments are the paper's statement of the problem

@@ -54,7 +54,7 @@ class MlStats(C.Structure):
     _fields_ = [
         ("rays_shot", C.c_uint64), ("rays_in_map", C.c_uint64), ("rays_dropped", C.c_uint64),
         ("interactions", C.c_uint64), ("kernel_launches", C.c_uint64),
-        ("kernel_ms", C.c_double), ("total_ms", C.c_double),
+        ("kernel_ms", C.c_double), ("total_ms", C.c_double), ("capture_ctas", C.c_uint64),
     ]
 
 
@@ -77,7 +77,8 @@ _lib = None
 
 
 def library_path() -> str:
-    return _build.LIB_PATH
+    """The in-tree library, or the build MICROLENS_B200_LIBRARY points at (a test build of the same sources)."""
+    return os.environ.get("MICROLENS_B200_LIBRARY") or _build.LIB_PATH
 
 
 def load():
@@ -85,8 +86,11 @@ def load():
     global _lib
     if _lib is not None:
         return _lib
-    path = _build.LIB_PATH
-    if _build.is_stale():
+    path = library_path()
+    if path != _build.LIB_PATH:
+        if not os.path.exists(path):
+            raise RuntimeError("MICROLENS_B200_LIBRARY=%s does not exist (there is no CPU fallback)" % path)
+    elif _build.is_stale():
         try:
             _build.build_library()
         except Exception as e:  # no nvcc on this box: use the shipped .so if there is one

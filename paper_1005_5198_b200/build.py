@@ -38,19 +38,24 @@ def is_stale() -> bool:
     return any(os.path.getmtime(s) > t for s in DEPENDS)
 
 
-def build_library(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/*.cu into libmicrolens_b200.so next to this file; returns its path."""
-    if not force and not is_stale():
+def build_library(force: bool = False, verbose: bool = False, defines=(), out: str = None) -> str:
+    """Compile csrc/*.cu into libmicrolens_b200.so next to this file; returns its path.
+
+    `defines` (e.g. ["ML_MAX_GRID_Y=50"]) and `out` make a separate TEST build of the same sources (the
+    launch-split test uses one); such a build is loaded by pointing MICROLENS_B200_LIBRARY at it (binding.load)."""
+    target = out or LIB_PATH
+    if not out and not defines and not force and not is_stale():
         return LIB_PATH
-    tmp = LIB_PATH + ".tmp%d" % os.getpid()
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
+    tmp = target + ".tmp%d" % os.getpid()
+    cmd = ([_nvcc()] + NVCC_FLAGS + ["-D" + d for d in defines] + (["-Xptxas", "-v"] if verbose else [])
+           + ["-o", tmp] + SOURCES)
     try:
         subprocess.check_call(cmd, cwd=_HERE)
-        os.replace(tmp, LIB_PATH)
+        os.replace(tmp, target)
     finally:
         if os.path.exists(tmp):
             os.remove(tmp)
-    return LIB_PATH
+    return target
 
 
 if __name__ == "__main__":

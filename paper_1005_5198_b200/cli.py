@@ -8,8 +8,10 @@ the computation runs in the CUDA library).
 The arguments are the paper's statement of the problem.  Lens positions are read from a
 text file of "x y" pairs in Einstein radii (the paper reads them from a file too) or, without one,
 drawn uniformly in the lens disk of radius R* with numpy's PCG64 and the given seed.  --out writes the raw uint32
-counts N_ij (mu_ij = N_ij / N_rays, eq. 3); --pgm writes an 8-bit greyscale picture of Delta m = -2.5 log10(mu / mu_th)
-like the paper's Fig. 1.
+counts N_ij (mu_ij = N_ij / N_rays, eq. 3); --pgm writes an 8-bit greyscale picture like the paper's Fig. 1
+(PAPER.md:23-25).  The picture is PRESENTATION ONLY: its grey levels are a numpy rendering of the counts on the host
+(Delta m of eq. 10 clipped to +-3 mag); the method's own Delta m statistics (histogram, RMS, K-S test) are the library
+calls ml_delta_m_histogram / ml_map_compare, and --dm-hist prints the former.
 """
 from __future__ import annotations
 
@@ -26,10 +28,13 @@ PRECISIONS = {"fp32_tiled": _b.ML_PREC_FP32_TILED, "fp32_compensated": _b.ML_PRE
 
 
 def _disk(n, radius, seed):
-    rng = np.random.default_rng(seed)
-    u, v = rng.random(n), rng.random(n)
-    r, th = radius * np.sqrt(u), 2.0 * np.pi * v
-    return np.stack([r * np.cos(th), r * np.sin(th)], axis=1)
+    """The repo's seeded synthetic lens field (workloads/lens_fields.py: the stand-in for the paper's lens files)."""
+    import os
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    if root not in sys.path:
+        sys.path.insert(0, root)
+    from workloads import lens_disk
+    return lens_disk(n, radius, seed)
 
 
 def main(argv=None) -> int:
@@ -47,7 +52,9 @@ def main(argv=None) -> int:
     ap.add_argument("--random-rays", type=int, default=None, metavar="SEED", help="random ray positions (GPU-D's way)")
     ap.add_argument("--device", type=int, default=0)
     ap.add_argument("--out", help="write the uint32 counts to this .npy file")
-    ap.add_argument("--pgm", help="write a greyscale picture of Delta m to this .pgm file")
+    ap.add_argument("--pgm", help="write a greyscale picture of Delta m to this .pgm file (presentation only)")
+    ap.add_argument("--dm-hist", type=int, default=0, metavar="BINS",
+                    help="print the Delta m histogram over [-3, 3) mag relative to mu_th (ml_delta_m_histogram)")
     a = ap.parse_args(argv)
 
     with MagnificationMap(a.sigma, a.stellar_fraction, a.gamma, a.n_pix, a.n_rays, a.L, device=a.device,
@@ -65,6 +72,12 @@ def main(argv=None) -> int:
                                                                   st["rays_in_map"], st["rays_dropped"]))
     print("kernel %.3f ms  %.4e lens-ray interactions/s  mean mu %.5f  (1/((1-sigma)^2-gamma^2) = %.5f)"
           % (st["kernel_ms"], st["interactions"] / max(st["kernel_ms"], 1e-9) * 1e3, mu_mean, info["mu_theory"]))
+    if a.dm_hist > 0:
+        # Delta m relative to the theoretical mean: count / (n_rays |mu_th|)
+        h = _b.ml_delta_m_histogram(counts, a.n_rays * abs(info["mu_theory"]), -3.0, 3.0, a.dm_hist, device=a.device)
+        w = 6.0 / a.dm_hist
+        for k, v in enumerate(h):
+            print("dm [%+.3f, %+.3f)  %d" % (-3.0 + k * w, -3.0 + (k + 1) * w, int(v)))
     if a.out:
         np.save(a.out, counts)
     if a.pgm:

@@ -11,16 +11,26 @@
 // is evaluated at the sample points of both maps (x = c/n_rays_a and x = c/n_rays_b, compared in
 // mu, which orders the samples exactly as Delta m does, reversed).  All sums that feed a
 // floating-point result are reduced in a fixed order: results are bit-reproducible.
+//
+// The magnitude difference of a pixel needs no logarithm table: with integer counts N_a, N_b
+//   dm_a - dm_b = -2.5 log10(N_a/N_b) + 2.5 log10(n_rays_a/n_rays_b),   ln(N_a/N_b) = 2 atanh(s),  s = (N_a - N_b)/(N_a + N_b)
+// (numerator and denominator exact), and the atanh series in s^2 needs 5-14 terms for maps that resemble each other
+// (|s| <= 1/4); a warp with a less similar pixel pair falls back to two fp64 logarithms per pixel.
+//
+// Host side: nothing is allocated, created or synchronised per call beyond the one read-back of the result; the
+// scratch (histograms, scans, events, a pinned result) lives in a per-device cache that grows when needed.
 #include "../../include/microlens.h"
 
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
 
+#include <mutex>
+
 namespace mlstats {
 
 constexpr int kThreads = 256;
-constexpr unsigned int kCap0 = 1u << 20;  // bins of the first-pass count histograms
+constexpr unsigned int kCap0 = 1u << 18;  // bins of the count histograms a scratch starts with (it grows on overflow)
 constexpr unsigned int kCapMax = 1u << 27;
 constexpr int kScanItems = 16;            // elements per thread in the scan kernels
 constexpr int kScanTile = kThreads * kScanItems;
@@ -31,37 +41,49 @@ struct Partial {
     unsigned int max_a, max_b;
 };
 
+// Device-resident state of one call, filled by reduce_partials_kernel and read by the kernels after it.
+struct Totals {
+    Partial t;
+    unsigned int cap_eff;  // max count + 1, clipped to the histogram size: the bins that matter
+    unsigned int overflow; // a count did not fit the histogram: the host repeats the call with more bins
+};
+
 constexpr int kPassThreads = 1024;        // one CTA per SM
 constexpr unsigned int kShBins = 16384;   // per map: counts below this are histogrammed in shared memory
-constexpr unsigned int kLut = 8192;       // log10(c) for c < kLut is tabulated per CTA in shared memory
+
+__constant__ double c_odd_recip[16] = {1.0, 1.0 / 3, 1.0 / 5, 1.0 / 7, 1.0 / 9, 1.0 / 11, 1.0 / 13, 1.0 / 15,
+                                       1.0 / 17, 1.0 / 19, 1.0 / 21, 1.0 / 23, 1.0 / 25, 1.0 / 27, 1.0 / 29, 1.0 / 31};
 
 __device__ __forceinline__ void hist_add(unsigned int *sh, unsigned int *hist, unsigned int cap, unsigned int c)
 {
-    if (c < kShBins) {
-        atomicAdd(&sh[c], 1u);
-    } else if (c < cap) {
-        // rare, bright pixels: warp-aggregated RED into the global histogram
-        const unsigned int peers = __match_any_sync(__activemask(), c);
-        if ((__ffs(peers) - 1) == (int)(threadIdx.x & 31)) atomicAdd(&hist[c], (unsigned int)__popc(peers));
-    }
+    if (c < kShBins) atomicAdd(&sh[c], 1u);
+    else if (c < cap) atomicAdd(&hist[c], 1u); // bright pixels: RED into the global histogram (L2)
+}
+
+// 1/d for an integer-valued d in [1, 2^33]: MUFU.RCP64H seed + two Newton-Raphson steps (relative error ~2^-52).
+__device__ __forceinline__ double recip_int(double d)
+{
+    double x;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
+    double e = __fma_rn(-d, x, 1.0);
+    x = __fma_rn(x, e, x);
+    e = __fma_rn(-d, x, 1.0);
+    return __fma_rn(x, e, x);
 }
 
 // One pass over the maps: RMS sums, statistics, count histograms (privatised per CTA in shared memory for
-// counts < kShBins, flushed once at the end).  STATS = false: histograms only (second pass when a count
-// exceeded the first-pass bins).
-template <bool TWO, bool STATS>
+// counts < kShBins, flushed once at the end).  TWO = false: one map (ml_delta_m_histogram).
+template <bool TWO>
 __global__ void __launch_bounds__(kPassThreads, 1) pass_kernel(const unsigned int *__restrict__ a, const unsigned int *__restrict__ b,
                                                                long long n, double n_rays_a, double n_rays_b, unsigned int *hist_a,
                                                                unsigned int *hist_b, unsigned int cap, Partial *partials)
 {
-    extern __shared__ __align__(8) unsigned char sh_raw[]; // [kLut] doubles, then [kShBins] bins for a and for b
-    double *sh_log = reinterpret_cast<double *>(sh_raw);
-    unsigned int *sh_hist = reinterpret_cast<unsigned int *>(sh_raw + kLut * sizeof(double));
+    extern __shared__ __align__(8) unsigned int sh_hist[]; // [kShBins] bins for a, then for b
     unsigned int *sh_a = sh_hist, *sh_b = sh_hist + kShBins;
     for (unsigned int k = threadIdx.x; k < (TWO ? 2 : 1) * kShBins; k += kPassThreads) sh_hist[k] = 0u;
-    if (TWO && STATS)
-        for (unsigned int k = threadIdx.x; k < kLut; k += kPassThreads) sh_log[k] = log10((double)k); // [0] = -inf, never read
-    const double log_rays = (n_rays_a == n_rays_b) ? 0.0 : log10(n_rays_a / n_rays_b);
+    // dm_a - dm_b = kLn * ln(N_a/N_b) + kRays   (eq. 10), kLn = -2.5/ln 10, kRays = 2.5 log10(n_rays_a/n_rays_b)
+    const double kLn = -2.5 / 2.302585092994046;
+    const double kRays = (n_rays_a == n_rays_b) ? 0.0 : 2.5 * log10(n_rays_a / n_rays_b);
     __syncthreads();
 
     Partial p;
@@ -72,87 +94,93 @@ __global__ void __launch_bounds__(kPassThreads, 1) pass_kernel(const unsigned in
     const long long stride = (long long)gridDim.x * kPassThreads * 4;
     unsigned int n_valid = 0, n_empty_a = 0, n_empty_b = 0; // per thread: < 2^31 / (gridDim.x * 1024) pixels each
 
-    auto load4 = [&](long long i, unsigned int (&ca)[4], unsigned int (&cb)[4]) {
+    auto load4 = [&](long long i, unsigned int (&ca)[4], unsigned int (&cb)[4], int &cnt) {
 #pragma unroll
         for (int q = 0; q < 4; ++q) { ca[q] = 0u; cb[q] = 0u; }
-        if (i >= n) return;
-        if (vec && i + 3 < n) {
-            const uint4 va = *reinterpret_cast<const uint4 *>(a + i);
+        cnt = i < n ? (int)min(4ll, n - i) : 0;
+        if (cnt == 4 && vec) {
+            const uint4 va = __ldcs(reinterpret_cast<const uint4 *>(a + i)); // streamed: read once
             ca[0] = va.x; ca[1] = va.y; ca[2] = va.z; ca[3] = va.w;
             if (TWO) {
-                const uint4 vb = *reinterpret_cast<const uint4 *>(b + i);
+                const uint4 vb = __ldcs(reinterpret_cast<const uint4 *>(b + i));
                 cb[0] = vb.x; cb[1] = vb.y; cb[2] = vb.z; cb[3] = vb.w;
             }
         } else {
 #pragma unroll
             for (int q = 0; q < 4; ++q)
-                if (i + q < n) {
+                if (q < cnt) {
                     ca[q] = a[i + q];
                     if (TWO) cb[q] = b[i + q];
                 }
         }
     };
-    auto process4 = [&](long long i, const unsigned int (&ca)[4], const unsigned int (&cb)[4]) {
-        if (i >= n) return;
-        const unsigned int big = ca[0] | ca[1] | ca[2] | ca[3] | cb[0] | cb[1] | cb[2] | cb[3];
-        if (i + 3 < n && big < kLut) {
-            // common case: four pixels, every count inside the log table and the shared-memory bins: no range checks
-            unsigned int s_a = 0, s_b = 0;
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                atomicAdd(&sh_a[ca[q]], 1u);
-                if (TWO) atomicAdd(&sh_b[cb[q]], 1u);
-                if (STATS) {
-                    s_a += ca[q];
-                    p.max_a = max(p.max_a, ca[q]);
-                    n_empty_a += (ca[q] == 0);
-                    if (TWO) {
-                        s_b += cb[q];
-                        p.max_b = max(p.max_b, cb[q]);
-                        n_empty_b += (cb[q] == 0);
-                        const bool valid = (ca[q] != 0) & (cb[q] != 0);
-                        // dm_a - dm_b = -2.5 (log10 N_a - log10 N_b - log10(n_rays_a / n_rays_b))   (eq. 10)
-                        const double d = -2.5 * ((sh_log[ca[q]] - sh_log[cb[q]]) - log_rays);
-                        p.ssq += valid ? d * d : 0.0;
-                        n_valid += valid;
-                    }
-                }
-            }
-            p.sum_a += s_a;
-            p.sum_b += s_b;
-            return;
-        }
+    // every thread of the CTA runs the same number of iterations (warp-wide votes inside): cnt = 0 means "no pixels"
+    auto process4 = [&](const unsigned int (&ca)[4], const unsigned int (&cb)[4], int cnt) {
+        unsigned int s_a = 0, s_b = 0;
+        double sv[4];
+        float s2max = 0.f;
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
-            if (i + q >= n) break;
-            hist_add(sh_a, hist_a, cap, ca[q]);
-            if (TWO) hist_add(sh_b, hist_b, cap, cb[q]);
-            if (STATS) {
-                p.sum_a += ca[q];
-                p.max_a = max(p.max_a, ca[q]);
-                n_empty_a += (ca[q] == 0);
-                if (TWO) {
-                    p.sum_b += cb[q];
-                    p.max_b = max(p.max_b, cb[q]);
-                    n_empty_b += (cb[q] == 0);
-                    if (ca[q] > 0 && cb[q] > 0) {
-                        const double la = ca[q] < kLut ? sh_log[ca[q]] : log10((double)ca[q]);
-                        const double lb = cb[q] < kLut ? sh_log[cb[q]] : log10((double)cb[q]);
-                        const double d = -2.5 * ((la - lb) - log_rays);
-                        p.ssq += d * d;
-                        n_valid += 1;
-                    }
-                }
+            const bool live = q < cnt;
+            if (live) {
+                hist_add(sh_a, hist_a, cap, ca[q]);
+                if (TWO) hist_add(sh_b, hist_b, cap, cb[q]);
             }
+            s_a += ca[q]; // dead slots hold 0
+            p.max_a = max(p.max_a, ca[q]);
+            n_empty_a += live && (ca[q] == 0);
+            if (TWO) {
+                s_b += cb[q];
+                p.max_b = max(p.max_b, cb[q]);
+                n_empty_b += live && (cb[q] == 0);
+                const bool valid = (ca[q] != 0) & (cb[q] != 0);
+                n_valid += valid;
+                // s = (N_a - N_b)/(N_a + N_b): both exact in fp64; s = 0 for pixels outside the RMS (M1)
+                const double fa = (double)ca[q], fb = (double)cb[q];
+                const double num = fa - fb, den = valid ? fa + fb : 1.0;
+                const double r = recip_int(den);
+                double s = num * r;
+                s = __fma_rn(__fma_rn(-den, s, num), r, s); // one correction step: s within an ulp of num/den
+                sv[q] = valid ? s : 0.0;
+                s2max = fmaxf(s2max, (float)(sv[q] * sv[q]));
+            }
+        }
+        p.sum_a += s_a;
+        if (!TWO) return;
+        p.sum_b += s_b;
+        // how many terms of atanh(s)/s = sum_k s^(2k)/(2k+1) this WARP needs for a relative truncation error < 2^-54
+        // (tail < s2^K/(1 - s2)): s2 <= 2^-12: 5, 2^-8: 7, 2^-6: 9, 2^-4: 14; beyond: two logarithms per pixel
+        const unsigned int key = __reduce_max_sync(0xffffffffu, __float_as_uint(s2max)); // s2 >= 0: bit order = value order
+        const float w = __uint_as_float(key);
+        if (w <= 0.0625f) {
+            const int K = w <= 0x1p-12f ? 5 : (w <= 0x1p-8f ? 7 : (w <= 0x1p-6f ? 9 : 14));
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const double s = sv[q], s2 = s * s;
+                double poly = c_odd_recip[K - 1];
+                for (int k = K - 2; k >= 0; --k) poly = __fma_rn(poly, s2, c_odd_recip[k]);
+                const double d = __fma_rn(kLn * 2.0, s * poly, kRays); // kLn ln(N_a/N_b) + kRays
+                p.ssq += (ca[q] != 0 && cb[q] != 0) ? d * d : 0.0;
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (ca[q] != 0 && cb[q] != 0) {
+                    const double d = __fma_rn(kLn, log((double)ca[q]) - log((double)cb[q]), kRays);
+                    p.ssq += d * d;
+                }
         }
     };
     // two quads in flight per thread: the loads of the second are issued before the first is processed
-    for (long long i = ((long long)blockIdx.x * kPassThreads + threadIdx.x) * 4; i < n; i += 2 * stride) {
+    const long long first = ((long long)blockIdx.x * kPassThreads + threadIdx.x) * 4;
+    const long long warp_first = ((long long)blockIdx.x * kPassThreads + (threadIdx.x & ~31)) * 4; // same for the whole warp
+    for (long long off = 0; warp_first + off < n; off += 2 * stride) {
         unsigned int ca0[4], cb0[4], ca1[4], cb1[4];
-        load4(i, ca0, cb0);
-        load4(i + stride, ca1, cb1);
-        process4(i, ca0, cb0);
-        process4(i + stride, ca1, cb1);
+        int c0, c1;
+        load4(first + off, ca0, cb0, c0);
+        load4(first + off + stride, ca1, cb1, c1);
+        process4(ca0, cb0, c0);
+        process4(ca1, cb1, c1);
     }
     p.n_valid = n_valid; p.n_empty_a = n_empty_a; p.n_empty_b = n_empty_b;
     __syncthreads();
@@ -164,32 +192,30 @@ __global__ void __launch_bounds__(kPassThreads, 1) pass_kernel(const unsigned in
             if (vb) atomicAdd(&hist_b[k], vb);
         }
     }
-    if constexpr (STATS) {
-        // block reduction in a fixed order: lanes by shuffle tree, then warps in index order
+    // block reduction in a fixed order: lanes by shuffle tree, then warps in index order
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            p.ssq += __shfl_down_sync(0xffffffffu, p.ssq, o);
-            p.n_valid += __shfl_down_sync(0xffffffffu, p.n_valid, o);
-            p.n_empty_a += __shfl_down_sync(0xffffffffu, p.n_empty_a, o);
-            p.n_empty_b += __shfl_down_sync(0xffffffffu, p.n_empty_b, o);
-            p.sum_a += __shfl_down_sync(0xffffffffu, p.sum_a, o);
-            p.sum_b += __shfl_down_sync(0xffffffffu, p.sum_b, o);
-            p.max_a = max(p.max_a, __shfl_down_sync(0xffffffffu, p.max_a, o));
-            p.max_b = max(p.max_b, __shfl_down_sync(0xffffffffu, p.max_b, o));
+    for (int o = 16; o > 0; o >>= 1) {
+        p.ssq += __shfl_down_sync(0xffffffffu, p.ssq, o);
+        p.n_valid += __shfl_down_sync(0xffffffffu, p.n_valid, o);
+        p.n_empty_a += __shfl_down_sync(0xffffffffu, p.n_empty_a, o);
+        p.n_empty_b += __shfl_down_sync(0xffffffffu, p.n_empty_b, o);
+        p.sum_a += __shfl_down_sync(0xffffffffu, p.sum_a, o);
+        p.sum_b += __shfl_down_sync(0xffffffffu, p.sum_b, o);
+        p.max_a = max(p.max_a, __shfl_down_sync(0xffffffffu, p.max_a, o));
+        p.max_b = max(p.max_b, __shfl_down_sync(0xffffffffu, p.max_b, o));
+    }
+    __shared__ Partial wp[kPassThreads / 32];
+    if ((threadIdx.x & 31) == 0) wp[threadIdx.x >> 5] = p;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        Partial t = wp[0];
+        for (int w = 1; w < kPassThreads / 32; ++w) {
+            t.ssq += wp[w].ssq;
+            t.n_valid += wp[w].n_valid; t.n_empty_a += wp[w].n_empty_a; t.n_empty_b += wp[w].n_empty_b;
+            t.sum_a += wp[w].sum_a; t.sum_b += wp[w].sum_b;
+            t.max_a = max(t.max_a, wp[w].max_a); t.max_b = max(t.max_b, wp[w].max_b);
         }
-        __shared__ Partial wp[kPassThreads / 32];
-        if ((threadIdx.x & 31) == 0) wp[threadIdx.x >> 5] = p;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            Partial t = wp[0];
-            for (int w = 1; w < kPassThreads / 32; ++w) {
-                t.ssq += wp[w].ssq;
-                t.n_valid += wp[w].n_valid; t.n_empty_a += wp[w].n_empty_a; t.n_empty_b += wp[w].n_empty_b;
-                t.sum_a += wp[w].sum_a; t.sum_b += wp[w].sum_b;
-                t.max_a = max(t.max_a, wp[w].max_a); t.max_b = max(t.max_b, wp[w].max_b);
-            }
-            partials[blockIdx.x] = t;
-        }
+        partials[blockIdx.x] = t;
     }
 }
 
@@ -202,7 +228,8 @@ __device__ __forceinline__ void add_partial(Partial &t, const Partial &q)
 }
 
 // Sum the per-block partials in a fixed order: one warp, lane l takes blocks l, l+32, ..., then a shuffle tree.
-__global__ void reduce_partials_kernel(const Partial *partials, int n_blocks, Partial *out)
+// Also fixes how many histogram bins the rest of the call has to look at.
+__global__ void reduce_partials_kernel(const Partial *partials, int n_blocks, unsigned int cap, Totals *out)
 {
     const int lane = threadIdx.x;
     Partial t;
@@ -223,17 +250,27 @@ __global__ void reduce_partials_kernel(const Partial *partials, int n_blocks, Pa
         q.max_b = __shfl_down_sync(0xffffffffu, t.max_b, o);
         add_partial(t, q);
     }
-    if (lane == 0) *out = t;
+    if (lane == 0) {
+        const unsigned int mx = max(t.max_a, t.max_b);
+        out->t = t;
+        out->overflow = mx >= cap ? 1u : 0u;
+        out->cap_eff = mx >= cap ? cap : mx + 1u;
+    }
 }
 
-// ---- inclusive prefix sums of a count histogram (three small kernels, tiles of kScanTile bins)
-__global__ void __launch_bounds__(kThreads) scan_tile_sums_kernel(const unsigned int *hist, unsigned int cap, unsigned int *tile_sums)
+// ---- inclusive prefix sums of the count histograms (three small kernels, tiles of kScanTile bins; blockIdx.y = map;
+//      the grids are sized for the whole histogram and blocks beyond cap_eff leave at once)
+__global__ void __launch_bounds__(kThreads) scan_tile_sums_kernel(const unsigned int *hist, unsigned int cap, const Totals *tot,
+                                                                  unsigned int *tile_sums, int n_tiles)
 {
+    const unsigned int cap_eff = tot->cap_eff;
     const unsigned int base = blockIdx.x * kScanTile;
+    if (base >= cap_eff) return;
+    hist += (size_t)blockIdx.y * cap;
     unsigned int s = 0;
     for (int q = 0; q < kScanItems; ++q) {
         const unsigned int k = base + q * kThreads + threadIdx.x;
-        if (k < cap) s += hist[k];
+        if (k < cap_eff) s += hist[k];
     }
     __shared__ unsigned int ws[kThreads / 32];
 #pragma unroll
@@ -243,31 +280,37 @@ __global__ void __launch_bounds__(kThreads) scan_tile_sums_kernel(const unsigned
     if (threadIdx.x == 0) {
         unsigned int t = 0;
         for (int w = 0; w < kThreads / 32; ++w) t += ws[w];
-        tile_sums[blockIdx.x] = t;
+        tile_sums[blockIdx.y * n_tiles + blockIdx.x] = t;
     }
 }
 
-__global__ void scan_tile_offsets_kernel(unsigned int *tile_sums, int n_tiles)
+__global__ void scan_tile_offsets_kernel(unsigned int *tile_sums, int n_tiles, const Totals *tot)
 {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    if (threadIdx.x != 0) return;
+    const int used = (int)((tot->cap_eff + kScanTile - 1) / kScanTile);
+    unsigned int *ts = tile_sums + blockIdx.x * n_tiles; // blockIdx.x = map
     unsigned int run = 0;
-    for (int k = 0; k < n_tiles; ++k) {
-        const unsigned int v = tile_sums[k];
-        tile_sums[k] = run; // exclusive
+    for (int k = 0; k < used; ++k) {
+        const unsigned int v = ts[k];
+        ts[k] = run; // exclusive
         run += v;
     }
 }
 
-__global__ void __launch_bounds__(kThreads) scan_apply_kernel(const unsigned int *hist, unsigned int cap, const unsigned int *tile_offsets,
-                                                              unsigned int *cum)
+__global__ void __launch_bounds__(kThreads) scan_apply_kernel(const unsigned int *hist, unsigned int cap, const Totals *tot,
+                                                              const unsigned int *tile_offsets, int n_tiles, unsigned int *cum)
 {
+    const unsigned int cap_eff = tot->cap_eff;
+    if (blockIdx.x * kScanTile >= cap_eff) return;
+    hist += (size_t)blockIdx.y * cap;
+    cum += (size_t)blockIdx.y * cap;
     // thread t owns the kScanItems consecutive bins starting at base + t*kScanItems
     const unsigned int base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
     unsigned int v[kScanItems];
     unsigned int s = 0;
 #pragma unroll
     for (int q = 0; q < kScanItems; ++q) {
-        v[q] = (base + q < cap) ? hist[base + q] : 0u;
+        v[q] = (base + q < cap_eff) ? hist[base + q] : 0u;
         s += v[q];
     }
     // exclusive scan of the per-thread sums over the block
@@ -281,13 +324,13 @@ __global__ void __launch_bounds__(kThreads) scan_apply_kernel(const unsigned int
     __shared__ unsigned int ws[kThreads / 32];
     if (lane == 31) ws[warp] = incl;
     __syncthreads();
-    unsigned int off = tile_offsets[blockIdx.x];
+    unsigned int off = tile_offsets[blockIdx.y * n_tiles + blockIdx.x];
     for (int w = 0; w < warp; ++w) off += ws[w];
     unsigned int run = off + incl - s;
 #pragma unroll
     for (int q = 0; q < kScanItems; ++q) {
         run += v[q];
-        if (base + q < cap) cum[base + q] = run;
+        if (base + q < cap_eff) cum[base + q] = run;
     }
 }
 
@@ -303,12 +346,14 @@ __device__ __forceinline__ unsigned int floor_ratio(unsigned int c, double num, 
 }
 
 // D = max_x |F_a(x) - F_b(x)| at the sample points of both maps (x in mu = count / n_rays).
-__global__ void __launch_bounds__(kThreads) ks_kernel(const unsigned int *cum_a, const unsigned int *cum_b, unsigned int cap, double n,
+__global__ void __launch_bounds__(kThreads) ks_kernel(const unsigned int *cum, unsigned int cap, const Totals *tot, double n,
                                                       double n_rays_a, double n_rays_b, unsigned long long *d_bits)
 {
+    const unsigned int cap_eff = tot->cap_eff;
+    const unsigned int *cum_a = cum, *cum_b = cum + cap;
     double d = 0.0;
-    const unsigned int last = cap - 1;
-    for (unsigned int c = blockIdx.x * kThreads + threadIdx.x; c < cap; c += gridDim.x * kThreads) {
+    const unsigned int last = cap_eff - 1;
+    for (unsigned int c = blockIdx.x * kThreads + threadIdx.x; c < cap_eff; c += gridDim.x * kThreads) {
         // x = c / n_rays_a : F_a = cum_a[c], F_b = #{N_b <= c n_rays_b / n_rays_a}
         const double fa1 = (double)cum_a[c] / n, fb1 = (double)cum_b[floor_ratio(c, n_rays_b, n_rays_a, last)] / n;
         // x = c / n_rays_b
@@ -321,11 +366,12 @@ __global__ void __launch_bounds__(kThreads) ks_kernel(const unsigned int *cum_a,
 }
 
 // Delta m histogram from the count histogram: one evaluation of eq. 10 per distinct count.
-__global__ void __launch_bounds__(kThreads) delta_m_hist_kernel(const unsigned int *hist, unsigned int cap, double n_rays, double lo, double hi,
+__global__ void __launch_bounds__(kThreads) delta_m_hist_kernel(const unsigned int *hist, const Totals *tot, double n_rays, double lo, double hi,
                                                                 int n_bins, unsigned long long *out)
 {
+    const unsigned int cap_eff = tot->cap_eff;
     const double w = (hi - lo) / (double)n_bins;
-    for (unsigned int c = 1 + blockIdx.x * kThreads + threadIdx.x; c < cap; c += gridDim.x * kThreads) {
+    for (unsigned int c = 1 + blockIdx.x * kThreads + threadIdx.x; c < cap_eff; c += gridDim.x * kThreads) {
         const unsigned int h = hist[c];
         if (!h) continue;
         const double x = -2.5 * log10((double)c / n_rays);
@@ -336,11 +382,11 @@ __global__ void __launch_bounds__(kThreads) delta_m_hist_kernel(const unsigned i
 }
 
 // Q_KS(lambda) = 2 sum_{j>=1} (-1)^(j-1) exp(-2 j^2 lambda^2), lambda = (sqrt(Ne) + 0.12 + 0.11/sqrt(Ne)) D.
-__global__ void finalize_kernel(const Partial *tot, const unsigned long long *d_bits, double n, double n_rays_a, double n_rays_b,
+__global__ void finalize_kernel(const Totals *tot, const unsigned long long *d_bits, double n, double n_rays_a, double n_rays_b,
                                 ml_map_compare_result *out)
 {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    const Partial t = *tot;
+    const Partial t = tot->t;
     ml_map_compare_result r;
     r.n_pixels = (uint64_t)n;
     r.n_valid = t.n_valid; r.n_empty_a = t.n_empty_a; r.n_empty_b = t.n_empty_b;
@@ -381,36 +427,106 @@ namespace {
 
 using namespace mlstats;
 
-struct StatsGuard { // device selection + everything the call allocates
+constexpr int kMaxDevices = 64;
+constexpr size_t kPassSmem = 2 * kShBins * sizeof(unsigned int);
+
+// Everything a call needs on one device, created on first use and kept: no allocation, event creation or
+// synchronisation per call besides the read-back of the result.  Calls are serialised by `lock` (a call ends with a
+// stream synchronisation, so the scratch is idle whenever the lock is free).
+struct Scratch {
+    bool ready = false;
+    int sm_count = 0;
+    unsigned int cap = 0;          // bins per histogram
+    unsigned char *zeroed = nullptr; // [2*cap hist | d_bits]: one memset per call
+    unsigned int *hist = nullptr;  // = zeroed: [2][cap]
+    unsigned long long *d_bits = nullptr;
+    unsigned long long *dm_out = nullptr; // [2^20] bins of ml_delta_m_histogram (allocated by its first call)
+    unsigned int *cum = nullptr;   // [2][cap]
+    unsigned int *tile_sums = nullptr; // [2][n_tiles]
+    Partial *partials = nullptr;   // [sm_count]
+    Totals *totals = nullptr;
+    ml_map_compare_result *d_res = nullptr;
+    struct Pinned { ml_map_compare_result res; Totals tot; } *pinned = nullptr;
+    unsigned int *map_a = nullptr, *map_b = nullptr; // device copies of host maps
+    size_t map_cap = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr, evp0 = nullptr, evp1 = nullptr; // whole call; the fused pass alone
+    void free_hist()
+    {
+        if (zeroed) cudaFree(zeroed);
+        if (cum) cudaFree(cum);
+        if (tile_sums) cudaFree(tile_sums);
+        zeroed = nullptr; cum = nullptr; tile_sums = nullptr; hist = nullptr; d_bits = nullptr;
+        cap = 0;
+    }
+    size_t zeroed_bytes(bool two) const { return two ? 2 * (size_t)cap * 4 + 8 : (size_t)cap * 4; }
+    int n_tiles() const { return (int)((cap + kScanTile - 1) / kScanTile); }
+    bool set_cap(unsigned int want)
+    {
+        if (want <= cap) return true;
+        free_hist();
+        cap = want;
+        if (cudaMalloc(&zeroed, zeroed_bytes(true)) != cudaSuccess || cudaMalloc(&cum, 2 * (size_t)cap * 4) != cudaSuccess ||
+            cudaMalloc(&tile_sums, 2 * (size_t)n_tiles() * 4) != cudaSuccess) {
+            cudaGetLastError();
+            free_hist();
+            return false;
+        }
+        hist = reinterpret_cast<unsigned int *>(zeroed);
+        d_bits = reinterpret_cast<unsigned long long *>(zeroed + 2 * (size_t)cap * 4);
+        return true;
+    }
+    bool set_maps(size_t n, bool two)
+    {
+        if (n <= map_cap && (!two || map_b)) return true;
+        if (map_a) cudaFree(map_a);
+        if (map_b) cudaFree(map_b);
+        map_a = map_b = nullptr;
+        map_cap = 0;
+        if (cudaMalloc(&map_a, n * 4) != cudaSuccess || cudaMalloc(&map_b, n * 4) != cudaSuccess) {
+            cudaGetLastError();
+            if (map_a) cudaFree(map_a);
+            map_a = map_b = nullptr;
+            return false;
+        }
+        map_cap = n;
+        return true;
+    }
+    int init(int device)
+    {
+        if (ready) return ML_OK;
+        if (cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return ML_ERR_CUDA;
+        if (cudaFuncSetAttribute(pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPassSmem) != cudaSuccess ||
+            cudaFuncSetAttribute(pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPassSmem) != cudaSuccess)
+            return ML_ERR_CUDA;
+        if (cudaMalloc(&partials, (size_t)sm_count * sizeof(Partial)) != cudaSuccess || cudaMalloc(&totals, sizeof(Totals)) != cudaSuccess ||
+            cudaMalloc(&d_res, sizeof(ml_map_compare_result)) != cudaSuccess || cudaMallocHost(&pinned, sizeof(Pinned)) != cudaSuccess) {
+            cudaGetLastError();
+            return ML_ERR_OOM;
+        }
+        if (cudaEventCreate(&ev0) != cudaSuccess || cudaEventCreate(&ev1) != cudaSuccess || cudaEventCreate(&evp0) != cudaSuccess ||
+            cudaEventCreate(&evp1) != cudaSuccess)
+            return ML_ERR_CUDA;
+        if (!set_cap(kCap0)) return ML_ERR_OOM;
+        ready = true;
+        return ML_OK;
+    }
+};
+
+Scratch g_scratch[kMaxDevices];
+std::mutex g_lock;
+
+struct DeviceScope { // device selection for the duration of a call
     int prev = 0;
     bool ok = false;
-    void *ptrs[20];
-    int n_ptrs = 0;
-    cudaEvent_t ev0 = nullptr, ev1 = nullptr, evp0 = nullptr, evp1 = nullptr; // whole call; the fused pass alone
-    cudaStream_t stream;
-    StatsGuard(int dev, cudaStream_t s) : stream(s)
+    explicit DeviceScope(int dev)
     {
         int ndev = 0;
-        if (cudaGetDeviceCount(&ndev) != cudaSuccess || dev < 0 || dev >= ndev) { cudaGetLastError(); return; }
+        if (cudaGetDeviceCount(&ndev) != cudaSuccess || dev < 0 || dev >= ndev || dev >= kMaxDevices) { cudaGetLastError(); return; }
         if (cudaGetDevice(&prev) != cudaSuccess) return;
         ok = (prev == dev) || (cudaSetDevice(dev) == cudaSuccess);
     }
-    template <typename T> T *alloc(size_t count)
+    ~DeviceScope()
     {
-        void *p = nullptr;
-        // stream-ordered allocation: no device-wide synchronisation per call
-        if (n_ptrs >= 20 || cudaMallocAsync(&p, (count ? count : 1) * sizeof(T), stream) != cudaSuccess) { cudaGetLastError(); return nullptr; }
-        ptrs[n_ptrs++] = p;
-        return static_cast<T *>(p);
-    }
-    ~StatsGuard()
-    {
-        for (int k = 0; k < n_ptrs; ++k) cudaFreeAsync(ptrs[k], stream);
-        if (ok && n_ptrs) cudaStreamSynchronize(stream);
-        if (ev0) cudaEventDestroy(ev0);
-        if (ev1) cudaEventDestroy(ev1);
-        if (evp0) cudaEventDestroy(evp0);
-        if (evp1) cudaEventDestroy(evp1);
         if (ok) cudaSetDevice(prev);
     }
 };
@@ -421,89 +537,41 @@ int grid_for(long long n, int sm_count)
     return (int)(want < 1 ? 1 : (want < sm_count ? want : sm_count)); // one CTA of 1024 threads per SM
 }
 
-constexpr size_t kPassSmem = kLut * sizeof(double) + 2 * kShBins * sizeof(unsigned int);
-
-template <bool TWO, bool STATS>
-cudaError_t launch_pass(int grid, cudaStream_t s, const unsigned int *a, const unsigned int *b, long long n, double na, double nb,
-                        unsigned int *ha, unsigned int *hb, unsigned int cap, Partial *partials)
+// Front half of both entry points: device copies of host maps, one memset, the fused pass, the reduced statistics.
+// Leaves Totals on the device (nothing is read back here).
+int run_pass(Scratch &sc, cudaStream_t s, const uint32_t *a, const uint32_t *b, int64_t n, double na, double nb, int where,
+             const unsigned int **da, const unsigned int **db)
 {
-    cudaError_t e = cudaFuncSetAttribute(pass_kernel<TWO, STATS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPassSmem);
-    if (e != cudaSuccess) return e;
-    pass_kernel<TWO, STATS><<<grid, kPassThreads, kPassSmem, s>>>(a, b, n, na, nb, ha, hb, cap, partials);
-    return cudaGetLastError();
-}
-
-// inclusive prefix sums of hist[0..cap) into cum[0..cap)
-bool scan_hist(const unsigned int *hist, unsigned int cap, unsigned int *tile_sums, unsigned int *cum, cudaStream_t s)
-{
-    const int n_tiles = (int)((cap + kScanTile - 1) / kScanTile);
-    scan_tile_sums_kernel<<<n_tiles, kThreads, 0, s>>>(hist, cap, tile_sums);
-    scan_tile_offsets_kernel<<<1, 32, 0, s>>>(tile_sums, n_tiles);
-    scan_apply_kernel<<<n_tiles, kThreads, 0, s>>>(hist, cap, tile_sums, cum);
-    return cudaGetLastError() == cudaSuccess;
-}
-
-// Shared front half of both entry points: device copies of the maps, the fused pass, the reduced
-// statistics on the host, and count histograms that hold every count (cap_eff bins used).
-struct PassOut {
-    const unsigned int *da = nullptr, *db = nullptr;
-    unsigned int *hist_a = nullptr, *hist_b = nullptr;
-    Partial *d_total = nullptr;
-    Partial total;
-    unsigned int cap_eff = 0;
-    int sm_count = 0;
-};
-
-int run_pass(StatsGuard &g, cudaStream_t s, const uint32_t *a, const uint32_t *b, int64_t n, double na, double nb, int where,
-             int device, PassOut &o)
-{
-    if (cudaDeviceGetAttribute(&o.sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return ML_ERR_CUDA;
     const bool two = b != nullptr;
-    o.da = a; o.db = b;
+    *da = a; *db = b;
     if (where == ML_MEM_HOST) {
-        unsigned int *ta = g.alloc<unsigned int>((size_t)n), *tb = two ? g.alloc<unsigned int>((size_t)n) : nullptr;
-        if (!ta || (two && !tb)) return ML_ERR_OOM;
-        if (cudaMemcpyAsync(ta, a, (size_t)n * 4, cudaMemcpyHostToDevice, s) != cudaSuccess ||
-            (two && cudaMemcpyAsync(tb, b, (size_t)n * 4, cudaMemcpyHostToDevice, s) != cudaSuccess))
+        if (!sc.set_maps((size_t)n, two)) return ML_ERR_OOM;
+        if (cudaMemcpyAsync(sc.map_a, a, (size_t)n * 4, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+            (two && cudaMemcpyAsync(sc.map_b, b, (size_t)n * 4, cudaMemcpyHostToDevice, s) != cudaSuccess))
             return ML_ERR_CUDA;
-        o.da = ta; o.db = tb;
+        *da = sc.map_a; *db = two ? sc.map_b : nullptr;
     }
-    const int grid = grid_for(n, o.sm_count);
-    Partial *partials = g.alloc<Partial>((size_t)grid);
-    o.d_total = g.alloc<Partial>(1);
-    o.hist_a = g.alloc<unsigned int>(kCap0);
-    o.hist_b = two ? g.alloc<unsigned int>(kCap0) : nullptr;
-    if (!partials || !o.d_total || !o.hist_a || (two && !o.hist_b)) return ML_ERR_OOM;
-    if (cudaEventCreate(&g.ev0) != cudaSuccess || cudaEventCreate(&g.ev1) != cudaSuccess || cudaEventCreate(&g.evp0) != cudaSuccess ||
-        cudaEventCreate(&g.evp1) != cudaSuccess)
+    const int grid = grid_for(n, sc.sm_count);
+    if (cudaEventRecord(sc.ev0, s) != cudaSuccess || cudaMemsetAsync(sc.zeroed, 0, sc.zeroed_bytes(two), s) != cudaSuccess ||
+        cudaEventRecord(sc.evp0, s) != cudaSuccess)
         return ML_ERR_CUDA;
-    if (cudaEventRecord(g.ev0, s) != cudaSuccess) return ML_ERR_CUDA;
-    if (cudaMemsetAsync(o.hist_a, 0, kCap0 * 4ull, s) != cudaSuccess || (two && cudaMemsetAsync(o.hist_b, 0, kCap0 * 4ull, s) != cudaSuccess))
-        return ML_ERR_CUDA;
-    if (cudaEventRecord(g.evp0, s) != cudaSuccess) return ML_ERR_CUDA;
-    if ((two ? launch_pass<true, true>(grid, s, o.da, o.db, n, na, nb, o.hist_a, o.hist_b, kCap0, partials)
-             : launch_pass<false, true>(grid, s, o.da, nullptr, n, na, nb, o.hist_a, nullptr, kCap0, partials)) != cudaSuccess)
-        return ML_ERR_CUDA;
-    if (cudaEventRecord(g.evp1, s) != cudaSuccess) return ML_ERR_CUDA;
-    reduce_partials_kernel<<<1, 32, 0, s>>>(partials, grid, o.d_total);
-    if (cudaGetLastError() != cudaSuccess) return ML_ERR_CUDA;
-    if (cudaMemcpyAsync(&o.total, o.d_total, sizeof(Partial), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
-        return ML_ERR_CUDA;
-    const unsigned int mx = o.total.max_a > o.total.max_b ? o.total.max_a : o.total.max_b;
-    if (mx >= kCapMax) return ML_ERR_OOM;
-    o.cap_eff = mx + 1;
-    if (o.cap_eff > kCap0) { // a count beyond the first-pass bins: histogram again with enough of them
-        o.hist_a = g.alloc<unsigned int>(o.cap_eff);
-        o.hist_b = two ? g.alloc<unsigned int>(o.cap_eff) : nullptr;
-        if (!o.hist_a || (two && !o.hist_b)) return ML_ERR_OOM;
-        if (cudaMemsetAsync(o.hist_a, 0, (size_t)o.cap_eff * 4, s) != cudaSuccess ||
-            (two && cudaMemsetAsync(o.hist_b, 0, (size_t)o.cap_eff * 4, s) != cudaSuccess))
-            return ML_ERR_CUDA;
-        if ((two ? launch_pass<true, false>(grid, s, o.da, o.db, n, na, nb, o.hist_a, o.hist_b, o.cap_eff, nullptr)
-                 : launch_pass<false, false>(grid, s, o.da, nullptr, n, na, nb, o.hist_a, nullptr, o.cap_eff, nullptr)) != cudaSuccess)
-            return ML_ERR_CUDA;
-    }
-    return ML_OK;
+    if (two) pass_kernel<true><<<grid, kPassThreads, kPassSmem, s>>>(*da, *db, n, na, nb, sc.hist, sc.hist + sc.cap, sc.cap, sc.partials);
+    else pass_kernel<false><<<grid, kPassThreads, kPassSmem, s>>>(*da, nullptr, n, na, nb, sc.hist, nullptr, sc.cap, sc.partials);
+    if (cudaGetLastError() != cudaSuccess || cudaEventRecord(sc.evp1, s) != cudaSuccess) return ML_ERR_CUDA;
+    reduce_partials_kernel<<<1, 32, 0, s>>>(sc.partials, grid, sc.cap, sc.totals);
+    return cudaGetLastError() == cudaSuccess ? ML_OK : ML_ERR_CUDA;
+}
+
+// After an overflow (a count >= the histogram size) the call is repeated once with enough bins.
+bool grow_after_overflow(Scratch &sc, const Totals &t, int *rc)
+{
+    if (!t.overflow) return false;
+    const unsigned int mx = t.t.max_a > t.t.max_b ? t.t.max_a : t.t.max_b;
+    if (mx >= kCapMax) { *rc = ML_ERR_OOM; return false; }
+    unsigned int want = sc.cap;
+    while (want <= mx) want *= 2;
+    if (!sc.set_cap(want)) { *rc = ML_ERR_OOM; return false; }
+    return true;
 }
 
 bool bad_rays(double v) { return !(v > 0.0) || !isfinite(v); }
@@ -519,28 +587,36 @@ int ml_map_compare(const uint32_t *a, double n_rays_a, const uint32_t *b, double
         (where != ML_MEM_HOST && where != ML_MEM_DEVICE))
         return ML_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    StatsGuard g(device, s);
+    DeviceScope g(device);
     if (!g.ok) return ML_ERR_CUDA;
-    PassOut o;
-    int rc = run_pass(g, s, a, b, n, n_rays_a, n_rays_b, where, device, o);
+    std::lock_guard<std::mutex> hold(g_lock);
+    Scratch &sc = g_scratch[device];
+    int rc = sc.init(device);
     if (rc != ML_OK) return rc;
-    const int n_tiles = (int)((o.cap_eff + kScanTile - 1) / kScanTile);
-    unsigned int *cum_a = g.alloc<unsigned int>(o.cap_eff), *cum_b = g.alloc<unsigned int>(o.cap_eff);
-    unsigned int *tiles = g.alloc<unsigned int>((size_t)n_tiles);
-    unsigned long long *d_bits = g.alloc<unsigned long long>(1);
-    ml_map_compare_result *d_res = g.alloc<ml_map_compare_result>(1);
-    if (!cum_a || !cum_b || !tiles || !d_bits || !d_res) return ML_ERR_OOM;
-    if (cudaMemsetAsync(d_bits, 0, 8, s) != cudaSuccess) return ML_ERR_CUDA;
-    if (!scan_hist(o.hist_a, o.cap_eff, tiles, cum_a, s) || !scan_hist(o.hist_b, o.cap_eff, tiles, cum_b, s)) return ML_ERR_CUDA;
-    const int ks_grid = (int)((o.cap_eff + kThreads - 1) / kThreads) < o.sm_count * 8 ? (int)((o.cap_eff + kThreads - 1) / kThreads) : o.sm_count * 8;
-    ks_kernel<<<ks_grid, kThreads, 0, s>>>(cum_a, cum_b, o.cap_eff, (double)n, n_rays_a, n_rays_b, d_bits);
-    finalize_kernel<<<1, 32, 0, s>>>(o.d_total, d_bits, (double)n, n_rays_a, n_rays_b, d_res);
-    if (cudaGetLastError() != cudaSuccess || cudaEventRecord(g.ev1, s) != cudaSuccess) return ML_ERR_CUDA;
-    if (cudaMemcpyAsync(out, d_res, sizeof(*out), cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
-        return ML_ERR_CUDA;
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        const unsigned int *da, *db;
+        rc = run_pass(sc, s, a, b, n, n_rays_a, n_rays_b, where, &da, &db);
+        if (rc != ML_OK) return rc;
+        const int n_tiles = sc.n_tiles();
+        scan_tile_sums_kernel<<<dim3(n_tiles, 2), kThreads, 0, s>>>(sc.hist, sc.cap, sc.totals, sc.tile_sums, n_tiles);
+        scan_tile_offsets_kernel<<<2, 32, 0, s>>>(sc.tile_sums, n_tiles, sc.totals);
+        scan_apply_kernel<<<dim3(n_tiles, 2), kThreads, 0, s>>>(sc.hist, sc.cap, sc.totals, sc.tile_sums, n_tiles, sc.cum);
+        const int want = (int)((sc.cap + kThreads - 1) / kThreads);
+        ks_kernel<<<want < sc.sm_count * 8 ? want : sc.sm_count * 8, kThreads, 0, s>>>(sc.cum, sc.cap, sc.totals, (double)n, n_rays_a, n_rays_b, sc.d_bits);
+        finalize_kernel<<<1, 32, 0, s>>>(sc.totals, sc.d_bits, (double)n, n_rays_a, n_rays_b, sc.d_res);
+        if (cudaGetLastError() != cudaSuccess || cudaEventRecord(sc.ev1, s) != cudaSuccess) return ML_ERR_CUDA;
+        if (cudaMemcpyAsync(&sc.pinned->res, sc.d_res, sizeof(ml_map_compare_result), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+            cudaMemcpyAsync(&sc.pinned->tot, sc.totals, sizeof(Totals), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+            cudaStreamSynchronize(s) != cudaSuccess)
+            return ML_ERR_CUDA;
+        if (grow_after_overflow(sc, sc.pinned->tot, &rc)) continue;
+        if (rc != ML_OK) return rc;
+        break;
+    }
     float ms = 0.f, pass_ms = 0.f;
-    if (cudaEventElapsedTime(&ms, g.ev0, g.ev1) != cudaSuccess || cudaEventElapsedTime(&pass_ms, g.evp0, g.evp1) != cudaSuccess)
+    if (cudaEventElapsedTime(&ms, sc.ev0, sc.ev1) != cudaSuccess || cudaEventElapsedTime(&pass_ms, sc.evp0, sc.evp1) != cudaSuccess)
         return ML_ERR_CUDA;
+    *out = sc.pinned->res;
     out->kernel_ms = ms;
     out->pass_kernel_ms = pass_ms;
     return ML_OK;
@@ -553,19 +629,33 @@ int ml_delta_m_histogram(const uint32_t *counts, double n_rays, int64_t n, doubl
         n_bins < 1 || n_bins > (1 << 20) || (where != ML_MEM_HOST && where != ML_MEM_DEVICE))
         return ML_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)cuda_stream;
-    StatsGuard g(device, s);
+    DeviceScope g(device);
     if (!g.ok) return ML_ERR_CUDA;
-    PassOut o;
-    int rc = run_pass(g, s, counts, nullptr, n, n_rays, n_rays, where, device, o);
+    std::lock_guard<std::mutex> hold(g_lock);
+    Scratch &sc = g_scratch[device];
+    int rc = sc.init(device);
     if (rc != ML_OK) return rc;
-    unsigned long long *d_out = g.alloc<unsigned long long>((size_t)n_bins);
-    if (!d_out) return ML_ERR_OOM;
-    if (cudaMemsetAsync(d_out, 0, (size_t)n_bins * 8, s) != cudaSuccess) return ML_ERR_CUDA;
-    const int want = (int)((o.cap_eff + kThreads - 1) / kThreads);
-    delta_m_hist_kernel<<<want < o.sm_count * 8 ? want : o.sm_count * 8, kThreads, 0, s>>>(o.hist_a, o.cap_eff, n_rays, lo, hi, n_bins, d_out);
-    if (cudaGetLastError() != cudaSuccess) return ML_ERR_CUDA;
-    if (cudaMemcpyAsync(hist_out, d_out, (size_t)n_bins * 8, cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess)
-        return ML_ERR_CUDA;
+    if (!sc.dm_out && cudaMalloc(&sc.dm_out, (size_t)(1 << 20) * 8) != cudaSuccess) {
+        cudaGetLastError();
+        sc.dm_out = nullptr;
+        return ML_ERR_OOM;
+    }
+    for (int attempt = 0; attempt < 2; ++attempt) {
+        const unsigned int *da, *db;
+        rc = run_pass(sc, s, counts, nullptr, n, n_rays, n_rays, where, &da, &db);
+        if (rc != ML_OK) return rc;
+        if (cudaMemsetAsync(sc.dm_out, 0, (size_t)n_bins * 8, s) != cudaSuccess) return ML_ERR_CUDA;
+        const int want = (int)((sc.cap + kThreads - 1) / kThreads);
+        delta_m_hist_kernel<<<want < sc.sm_count * 8 ? want : sc.sm_count * 8, kThreads, 0, s>>>(sc.hist, sc.totals, n_rays, lo, hi, n_bins, sc.dm_out);
+        if (cudaGetLastError() != cudaSuccess) return ML_ERR_CUDA;
+        if (cudaMemcpyAsync(hist_out, sc.dm_out, (size_t)n_bins * 8, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+            cudaMemcpyAsync(&sc.pinned->tot, sc.totals, sizeof(Totals), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+            cudaStreamSynchronize(s) != cudaSuccess)
+            return ML_ERR_CUDA;
+        if (grow_after_overflow(sc, sc.pinned->tot, &rc)) continue;
+        if (rc != ML_OK) return rc;
+        break;
+    }
     return ML_OK;
 }
 

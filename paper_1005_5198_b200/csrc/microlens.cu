@@ -32,7 +32,10 @@ struct ml_ctx {
     double2 *lens;
     double *mass;     // device masses m_i (eq.4), nullptr = unit masses
     int64_t n_lenses; // -1: never set
-    unsigned long long *counters; // device [3]
+    unsigned long long *counters; // device [3]: running totals, never reset (a shoot reports the difference)
+    unsigned long long *h_counters; // pinned host copy of the same
+    unsigned long long seen[3];     // device totals after the last shoot
+    unsigned long long base[3];     // device totals when the current (non-accumulating) run began
     int precision;
     int ray_mode;            // ML_RAYS_*
     unsigned long long ray_seed;
@@ -61,11 +64,11 @@ struct Mode {
 };
 constexpr int RXF = 4, RYF = 4, KFF = 64;  // FP32_TILED (shoot_kernel_pipe) and FP32_COMPENSATED
 constexpr int WARPS_T = 4, SHARED_T = 4, MINB_T = 3; // FP32_TILED: 128-thread CTAs, 3 per SM, all rows share
-constexpr int KFC = 8;                     // FP32_COMPENSATED, generic kernel (random rays)
 constexpr int KFCP = 16;                   // FP32_COMPENSATED, regular grid: the pipe kernel with a Newton step
 constexpr int RXD = 4, RYD = 2, KFD = 64;  // FP64
 
-constexpr int RXR = 4, RYR = 2;            // FP32 modes with random rays: every ray carries its own offsets
+constexpr int RXR = 4, RYR = kRandRY;      // FP32 modes with random rays (shoot_kernel_rpipe): every ray carries its own offsets
+static_assert(kRandWarps == kWarps, "mode_of: the random-ray kernels use 256-thread CTAs");
 
 Mode mode_of(int precision, int ray_mode)
 {
@@ -76,7 +79,7 @@ Mode mode_of(int precision, int ray_mode)
 
 Mode mode_of(const ml_ctx *c) { return mode_of(c->precision, c->ray_mode); }
 
-template <bool CAPTURE, bool MASS> cudaError_t launch_m(int precision, unsigned int g, const ShootParams &p, cudaStream_t s)
+template <bool CAPTURE, bool MASS> cudaError_t launch_m(int precision, dim3 g, const ShootParams &p, cudaStream_t s)
 {
     switch (precision) {
     case ML_PREC_FP64:
@@ -92,28 +95,42 @@ template <bool CAPTURE, bool MASS> cudaError_t launch_m(int precision, unsigned 
     return cudaGetLastError();
 }
 
-// random ray positions (reading R17): the generic kernel with per-ray offsets
-template <bool CAPTURE, bool MASS> cudaError_t launch_r(int precision, unsigned int g, const ShootParams &p, cudaStream_t s)
+#ifndef ML_RPIPE_OWN
+#define ML_RPIPE_OWN 1 // see shoot_kernel_rpipe: own reciprocals on the last row of odd lenses
+#endif
+// random ray positions (reading R17): the packed random-ray kernel in the FP32 modes, the generic
+// kernel with per-ray offsets in fp64
+template <int KF, bool CAPTURE, bool MASS, bool NEWTON> cudaError_t launch_rpipe(dim3 g, const ShootParams &p, cudaStream_t s)
+{
+    constexpr size_t smem = rpipe_smem_bytes(MASS);
+    static bool opted_in = false; // more than 48 KB of dynamic shared memory needs the opt-in once per function
+    if (!opted_in) {
+        const cudaError_t e = cudaFuncSetAttribute(shoot_kernel_rpipe<KF, 2, CAPTURE, MASS, NEWTON, ML_RPIPE_OWN>,
+                                                   cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        opted_in = true;
+    }
+    shoot_kernel_rpipe<KF, 2, CAPTURE, MASS, NEWTON, ML_RPIPE_OWN><<<g, kRandWarps * 32, smem, s>>>(p);
+    return cudaGetLastError();
+}
+
+template <bool CAPTURE, bool MASS> cudaError_t launch_r(int precision, dim3 g, const ShootParams &p, cudaStream_t s)
 {
     switch (precision) {
     case ML_PREC_FP64:
         shoot_kernel<double, RXD, RYD, KFD, false, CAPTURE, MASS, true><<<g, kThreads, 0, s>>>(p);
-        break;
+        return cudaGetLastError();
     case ML_PREC_FP32_COMPENSATED:
-        shoot_kernel<float, RXR, RYR, KFC, true, CAPTURE, MASS, true><<<g, kThreads, 0, s>>>(p);
-        break;
+        return launch_rpipe<KFCP, CAPTURE, MASS, true>(g, p, s);
     default:
-        shoot_kernel<float, RXR, RYR, KFF, false, CAPTURE, MASS, true><<<g, kThreads, 0, s>>>(p);
-        break;
+        return launch_rpipe<KFF, CAPTURE, MASS, false>(g, p, s);
     }
-    return cudaGetLastError();
 }
 
 // unit masses (every map of the paper) run the instantiations without the mass multiply
-template <bool CAPTURE> cudaError_t launch(int precision, int ray_mode, long long n_tiles, const ShootParams &p, cudaStream_t s)
+template <bool CAPTURE> cudaError_t launch(int precision, int ray_mode, dim3 g, const ShootParams &p, cudaStream_t s)
 {
-    if (n_tiles <= 0) return cudaSuccess;
-    const unsigned int g = (unsigned int)n_tiles;
+    if (g.x == 0 || g.y == 0) return cudaSuccess;
     if (ray_mode == ML_RAYS_RANDOM)
         return p.mass ? launch_r<CAPTURE, true>(precision, g, p, s) : launch_r<CAPTURE, false>(precision, g, p, s);
     return p.mass ? launch_m<CAPTURE, true>(precision, g, p, s) : launch_m<CAPTURE, false>(precision, g, p, s);
@@ -134,6 +151,9 @@ ShootParams base_params(const ml_ctx *c)
     p.c2 = 1.0 + c->gamma - c->kappa_c;
     p.halfL = c->L / 2.0;
     p.inv_pixel = (double)c->n_pix / c->L;
+    p.k1 = p.c1 * p.inv_pixel;
+    p.k2 = p.c2 * p.inv_pixel;
+    p.hoff = p.halfL * p.inv_pixel;
     p.map = c->map;
     p.counters = c->counters;
     p.n1 = c->n1;
@@ -141,7 +161,97 @@ ShootParams base_params(const ml_ctx *c)
     return p;
 }
 
-constexpr long long kMaxTilesPerLaunch = 0x7fffffffLL;
+// Second half of a split launch (see lens_range in shoot_kernel.cuh): add the partial sums of the lens ranges, then
+// write the positions (CAPTURE) or bin the rays.
+template <bool CAPTURE>
+cudaError_t launch_combine(int precision, int ray_mode, unsigned int n_tiles, const ShootParams &p, int n_splits, cudaStream_t s)
+{
+    const dim3 g(n_tiles, 1, 1);
+    if (precision == ML_PREC_FP64) {
+        if (ray_mode == ML_RAYS_RANDOM) combine_kernel<RXD, RYD, kWarps, true, CAPTURE><<<g, kThreads, 0, s>>>(p, n_splits);
+        else combine_kernel<RXD, RYD, kWarps, false, CAPTURE><<<g, kThreads, 0, s>>>(p, n_splits);
+    } else if (ray_mode == ML_RAYS_RANDOM) {
+        combine_kernel<RXR, RYR, kRandWarps, true, CAPTURE><<<g, kRandWarps * 32, 0, s>>>(p, n_splits);
+    } else {
+        combine_kernel<RXF, RYF, WARPS_T, false, CAPTURE><<<g, WARPS_T * 32, 0, s>>>(p, n_splits);
+    }
+    return cudaGetLastError();
+}
+
+// Lens ranges for a launch of nb tiles: none while the tiles alone give every SM work or the lens list is
+// short; otherwise enough ranges (multiples of the 512-lens chunk, at least 2048 lenses each) for about two CTAs
+// per SM, within `max_splits` (memory of the partial sums).
+int plan_lens_split(const ml_ctx *c, long long nb, long long max_splits, int *split_len)
+{
+    *split_len = 0;
+    const long long want_ctas = 2ll * c->sm_count;
+    if (c->n_lenses < 8192 || nb >= want_ctas || max_splits < 2) return 1;
+    long long splits = std::min<long long>({(want_ctas + nb - 1) / nb, c->n_lenses / 2048, max_splits});
+    if (splits < 2) return 1;
+    long long len = (c->n_lenses + splits - 1) / splits;
+    len = (len + kChunk - 1) / kChunk * kChunk;
+    splits = (c->n_lenses + len - 1) / len;
+    if (splits < 2) return 1;
+    *split_len = (int)len;
+    return (int)splits;
+}
+
+// ml_shoot_region over a handful of tiles and very many lenses: the capture instantiation (which bins nothing) runs
+// once per (tile, lens range) and leaves fp64 partial sums; combine_kernel<.., CAPTURE = false> adds them in range
+// order and bins the rays with the region masks.  Synchronises (the partial sums are freed before returning).
+int shoot_split(ml_ctx *c, ShootParams p, const Mode &m, long long ti0, long long tj0, long long tiles_x, long long tiles_y,
+                int n_splits, int split_len, float *ms)
+{
+    const long long n_tiles = tiles_x * tiles_y;
+    std::vector<long long> tiles;
+    try {
+        tiles.reserve((size_t)(2 * n_tiles));
+        for (long long ty = 0; ty < tiles_y; ++ty)
+            for (long long tx = 0; tx < tiles_x; ++tx) {
+                tiles.push_back(ti0 + tx);
+                tiles.push_back(tj0 + ty);
+            }
+    } catch (const std::bad_alloc &) {
+        return ML_ERR_OOM;
+    }
+    long long *d_list = nullptr;
+    double2 *d_part = nullptr;
+    int rc = ML_OK;
+    if (cudaMalloc(&d_list, tiles.size() * sizeof(long long)) != cudaSuccess ||
+        cudaMalloc(&d_part, (size_t)n_splits * n_tiles * m.tw * m.th * sizeof(double2)) != cudaSuccess) {
+        cudaGetLastError();
+        rc = ML_ERR_OOM;
+    }
+    if (rc == ML_OK) {
+        p.tile_list = d_list;
+        p.split_len = split_len;
+        p.partial = d_part;
+        if (cudaMemcpyAsync(d_list, tiles.data(), tiles.size() * sizeof(long long), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+            cudaEventRecord(c->ev0, c->stream) != cudaSuccess ||
+            launch<true>(c->precision, c->ray_mode, dim3((unsigned int)n_tiles, (unsigned int)n_splits, 1), p, c->stream) != cudaSuccess ||
+            launch_combine<false>(c->precision, c->ray_mode, (unsigned int)n_tiles, p, n_splits, c->stream) != cudaSuccess ||
+            cudaEventRecord(c->ev1, c->stream) != cudaSuccess || cudaStreamSynchronize(c->stream) != cudaSuccess ||
+            cudaEventElapsedTime(ms, c->ev0, c->ev1) != cudaSuccess)
+            rc = ML_ERR_CUDA;
+    }
+    if (d_list) cudaFree(d_list);
+    if (d_part) cudaFree(d_part);
+    if (rc == ML_OK) c->stats.capture_ctas = (uint64_t)n_tiles * (uint64_t)n_splits;
+    return rc;
+}
+
+// One shoot launch is a 2-D grid of tiles (x = tile column, y = tile row).  A grid holds at most 2^31 - 1 CTAs along x
+// and 65535 along y; larger regions are cut into several launches that continue the same tile raster (tile_i0 / tile_j0
+// of each launch).  The limits are macros so that a test build (-DML_MAX_GRID_X=7 -DML_MAX_GRID_Y=50) can exercise the
+// split on a small problem.
+#ifndef ML_MAX_GRID_X
+#define ML_MAX_GRID_X 0x7fffffffLL
+#endif
+#ifndef ML_MAX_GRID_Y
+#define ML_MAX_GRID_Y 65535LL
+#endif
+constexpr long long kMaxGridX = ML_MAX_GRID_X, kMaxGridY = ML_MAX_GRID_Y;
+static_assert(kMaxGridX >= 1 && kMaxGridX <= 0x7fffffffLL && kMaxGridY >= 1 && kMaxGridY <= 65535LL, "grid limits");
 
 int shoot_region_impl(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1, int accumulate)
 {
@@ -152,10 +262,11 @@ int shoot_region_impl(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1,
     if (!g.ok) return ML_ERR_CUDA;
     const auto t0 = std::chrono::steady_clock::now();
     if (!accumulate) {
-        if (cudaMemsetAsync(c->map, 0, (size_t)c->n_pix * c->n_pix * sizeof(unsigned int), c->stream) != cudaSuccess ||
-            cudaMemsetAsync(c->counters, 0, 3 * sizeof(unsigned long long), c->stream) != cudaSuccess)
+        // one memset: the counters are running totals and are never zeroed (the run's statistics are differences)
+        if (cudaMemsetAsync(c->map, 0, (size_t)c->n_pix * c->n_pix * sizeof(unsigned int), c->stream) != cudaSuccess)
             return ML_ERR_CUDA;
         std::memset(&c->stats, 0, sizeof(c->stats));
+        std::memcpy(c->base, c->seen, sizeof(c->base));
     }
     float ms = 0.f;
     uint64_t launches = 0;
@@ -163,29 +274,38 @@ int shoot_region_impl(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1,
         const Mode m = mode_of(c);
         ShootParams p = base_params(c);
         p.i0 = i0; p.i1 = i1; p.j0 = j0; p.j1 = j1;
-        p.tile_i0 = i0 / m.tw;
-        p.tile_j0 = j0 / m.th;
-        p.tiles_x = (i1 - 1) / m.tw - p.tile_i0 + 1;
-        const long long tiles_y = (j1 - 1) / m.th - p.tile_j0 + 1;
-        const long long n_tiles = p.tiles_x * tiles_y;
+        const long long ti0 = i0 / m.tw, tj0 = j0 / m.th;
+        const long long tiles_x = (i1 - 1) / m.tw - ti0 + 1, tiles_y = (j1 - 1) / m.th - tj0 + 1;
+        int split_len = 0;
+        const int n_splits = (double)tiles_x * (double)tiles_y < 4096.0
+                                 ? plan_lens_split(c, tiles_x * tiles_y, (1024ll << 20) / (tiles_x * tiles_y * m.tw * m.th * (long long)sizeof(double2)), &split_len)
+                                 : 1;
+        if (n_splits > 1) { // few rays, very many lenses: split the lens loop over CTAs, then combine and bin
+            const int rc = shoot_split(c, p, m, ti0, tj0, tiles_x, tiles_y, n_splits, split_len, &ms);
+            if (rc != ML_OK) return rc;
+            launches = 2;
+        } else {
         if (cudaEventRecord(c->ev0, c->stream) != cudaSuccess) return ML_ERR_CUDA;
-        for (long long base = 0; base < n_tiles; base += kMaxTilesPerLaunch) {
-            p.tile_base = base;
-            if (launch<false>(c->precision, c->ray_mode, std::min(kMaxTilesPerLaunch, n_tiles - base), p, c->stream) != cudaSuccess)
-                return ML_ERR_CUDA;
-            ++launches;
-        }
+        for (long long by = 0; by < tiles_y; by += kMaxGridY)
+            for (long long bx = 0; bx < tiles_x; bx += kMaxGridX) {
+                p.tile_i0 = ti0 + bx;
+                p.tile_j0 = tj0 + by;
+                const dim3 grid((unsigned int)std::min(kMaxGridX, tiles_x - bx), (unsigned int)std::min(kMaxGridY, tiles_y - by), 1);
+                if (launch<false>(c->precision, c->ray_mode, grid, p, c->stream) != cudaSuccess) return ML_ERR_CUDA;
+                ++launches;
+            }
         if (cudaEventRecord(c->ev1, c->stream) != cudaSuccess) return ML_ERR_CUDA;
+        }
     }
-    unsigned long long h[3];
-    if (cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+    if (cudaMemcpyAsync(c->h_counters, c->counters, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
         cudaStreamSynchronize(c->stream) != cudaSuccess)
         return ML_ERR_CUDA;
-    if (launches && cudaEventElapsedTime(&ms, c->ev0, c->ev1) != cudaSuccess) return ML_ERR_CUDA;
-    c->stats.rays_shot = h[0];
-    c->stats.rays_in_map = h[1];
-    c->stats.rays_dropped = h[2];
-    c->stats.interactions = h[0] * (uint64_t)c->n_lenses;
+    if (launches && ms == 0.f && cudaEventElapsedTime(&ms, c->ev0, c->ev1) != cudaSuccess) return ML_ERR_CUDA;
+    std::memcpy(c->seen, c->h_counters, sizeof(c->seen));
+    c->stats.rays_shot = c->seen[0] - c->base[0];
+    c->stats.rays_in_map = c->seen[1] - c->base[1];
+    c->stats.rays_dropped = c->seen[2] - c->base[2];
+    c->stats.interactions = c->stats.rays_shot * (uint64_t)c->n_lenses;
     c->stats.kernel_launches += launches;
     c->stats.kernel_ms += ms;
     c->stats.total_ms = std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - t0).count();
@@ -202,8 +322,10 @@ int capture_tiles(ml_ctx *c, const std::vector<long long> &tiles /* pairs */, Si
     const long long n_tiles = (long long)(tiles.size() / 2);
     if (n_tiles == 0) return ML_OK;
     const long long batch = std::max<long long>(1, std::min<long long>(n_tiles, (256ll << 20) / (long long)(per_tile * sizeof(double2))));
+    int split_len = 0;
+    const int n_splits = plan_lens_split(c, batch, (1024ll << 20) / (long long)(batch * per_tile * sizeof(double2)), &split_len);
     long long *d_list = nullptr;
-    double2 *d_buf = nullptr;
+    double2 *d_buf = nullptr, *d_part = nullptr;
     std::vector<double2> h_buf;
     try {
         h_buf.resize((size_t)batch * per_tile);
@@ -212,7 +334,8 @@ int capture_tiles(ml_ctx *c, const std::vector<long long> &tiles /* pairs */, Si
     }
     int rc = ML_OK;
     if (cudaMalloc(&d_list, tiles.size() * sizeof(long long)) != cudaSuccess ||
-        cudaMalloc(&d_buf, (size_t)batch * per_tile * sizeof(double2)) != cudaSuccess) {
+        cudaMalloc(&d_buf, (size_t)batch * per_tile * sizeof(double2)) != cudaSuccess ||
+        (n_splits > 1 && cudaMalloc(&d_part, (size_t)n_splits * batch * per_tile * sizeof(double2)) != cudaSuccess)) {
         cudaGetLastError();
         rc = ML_ERR_OOM;
     }
@@ -223,17 +346,27 @@ int capture_tiles(ml_ctx *c, const std::vector<long long> &tiles /* pairs */, Si
         ShootParams p = base_params(c);
         p.capture = d_buf;
         p.tile_list = d_list + 2 * first;
-        p.tile_base = 0;
-        if (launch<true>(c->precision, c->ray_mode, nb, p, c->stream) != cudaSuccess ||
+        cudaError_t e;
+        if (n_splits > 1) {
+            p.split_len = split_len;
+            p.partial = d_part;
+            e = launch<true>(c->precision, c->ray_mode, dim3((unsigned int)nb, (unsigned int)n_splits, 1), p, c->stream);
+            if (e == cudaSuccess) e = launch_combine<true>(c->precision, c->ray_mode, (unsigned int)nb, p, n_splits, c->stream);
+        } else {
+            e = launch<true>(c->precision, c->ray_mode, dim3((unsigned int)nb, 1, 1), p, c->stream);
+        }
+        if (e != cudaSuccess ||
             cudaMemcpyAsync(h_buf.data(), d_buf, (size_t)nb * per_tile * sizeof(double2), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
             cudaStreamSynchronize(c->stream) != cudaSuccess) {
             rc = ML_ERR_CUDA;
             break;
         }
+        c->stats.capture_ctas = n_splits > 1 ? (uint64_t)nb * (uint64_t)n_splits : 0;
         sink(first, nb, h_buf.data());
     }
     cudaFree(d_list);
     cudaFree(d_buf);
+    if (d_part) cudaFree(d_part);
     return rc;
 }
 
@@ -298,7 +431,8 @@ int ml_create(double sigma, double stellar_fraction, double gamma, int32_t n_pix
     if (rc == ML_OK) {
         c->stream = c->own_stream;
         if (cudaMalloc(&c->map_own, (size_t)n_pix * n_pix * sizeof(unsigned int)) != cudaSuccess ||
-            cudaMalloc(&c->counters, 3 * sizeof(unsigned long long)) != cudaSuccess) {
+            cudaMalloc(&c->counters, 3 * sizeof(unsigned long long)) != cudaSuccess ||
+            cudaMallocHost(&c->h_counters, 3 * sizeof(unsigned long long)) != cudaSuccess) {
             cudaGetLastError();
             rc = ML_ERR_OOM;
         }
@@ -329,6 +463,7 @@ void ml_destroy(ml_ctx *c)
             if (c->lens) cudaFree(c->lens);
             if (c->mass) cudaFree(c->mass);
             if (c->counters) cudaFree(c->counters);
+            if (c->h_counters) cudaFreeHost(c->h_counters);
             if (c->ev0) cudaEventDestroy(c->ev0);
             if (c->ev1) cudaEventDestroy(c->ev1);
             if (c->own_stream) cudaStreamDestroy(c->own_stream);
@@ -356,7 +491,7 @@ int ml_get_info(const ml_ctx *c, ml_info *o)
 
 int ml_set_lens_masses(ml_ctx *c, const double *xy, const double *mass, int64_t n)
 {
-    if (!c || n < 0 || n > 0x7fffff00LL || (n > 0 && !xy)) return ML_ERR_INVALID_ARG;
+    if (!c || n < 0 || n > 0x7ffffe00LL || (n > 0 && !xy)) return ML_ERR_INVALID_ARG; // base + 512 must fit an int in the kernels
     for (int64_t k = 0; k < 2 * n; ++k)
         if (!std::isfinite(xy[k])) return ML_ERR_INVALID_ARG;
     if (mass)

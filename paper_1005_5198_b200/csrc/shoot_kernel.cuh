@@ -24,8 +24,9 @@
 //
 // Summation order and precision:
 //   lenses in index order; FP32 partial sums over groups of KF consecutive lenses (groups
-//   aligned to multiples of KF in lens index) are added, in order, to one fp64
-//   accumulator per ray and component.  With Real = double the partials are fp64 too
+//   aligned to multiples of KF in lens index; a trailing group of fewer than KF/2 lenses is
+//   joined to the group before it when that group lies in the same 512-lens chunk) are added,
+//   in order, to one fp64 accumulator per ray and component.  With Real = double the partials are fp64 too
 //   and the reciprocal is an IEEE division.
 //   Every FP32 operation is written with an explicit-rounding intrinsic so that the
 //   compiler can neither contract nor reassociate: the arithmetic of a ray does not
@@ -33,6 +34,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <type_traits>
 
 namespace mlb200 {
 
@@ -42,17 +44,19 @@ struct ShootParams {
     int n_lens;
     int n_pix;
     long long i0, i1, j0, j1; // region of ray indices to count (others are masked)
-    long long tile_i0, tile_j0; // first global tile index along each axis for this launch
-    long long tiles_x;        // tiles per row of this launch
-    long long tile_base;      // added to blockIdx.x (launches of > 2^31-1 tiles are split)
+    long long tile_i0, tile_j0; // global tile index of block (0, 0) of this launch: tile = (tile_i0 + blockIdx.x,
+                              // tile_j0 + blockIdx.y); regions larger than one grid are split into several launches
     double delta;             // ray spacing
     double half1, half2;      // (n1-1)/2, (n2-1)/2
     double c1, c2;            // 1 - gamma - kappa_c, 1 + gamma - kappa_c
     double halfL, inv_pixel;  // L/2, n_pix/L
+    double k1, k2, hoff;      // c1 * inv_pixel, c2 * inv_pixel, halfL * inv_pixel: pixel coordinate u = k x + hoff - S inv_pixel
     unsigned int *map;        // [n_pix*n_pix] counts, device
     unsigned long long *counters; // [0] shot [1] in map [2] dropped
     double2 *capture;         // CAPTURE: [n_tiles_in_list * TW*TH] source-plane positions
     const long long *tile_list; // CAPTURE: pairs (tile_i, tile_j), global tile indices
+    int split_len;            // CAPTURE, > 0: CTA (t, blockIdx.y) sums lenses [blockIdx.y*split_len, +split_len) only
+    double2 *partial;         // CAPTURE with split_len > 0: [gridDim.y][gridDim.x][TW*TH] partial sums (Sx, Sy)
     long long n1;             // rays per row of the whole grid (ray id = j*n1 + i, RANDOM instantiations)
     unsigned long long ray_seed; // key of the ray generator (RANDOM instantiations)
 };
@@ -133,90 +137,210 @@ __device__ __forceinline__ void ray_uniforms(unsigned long long ray_id, unsigned
 
 // a4 + a5 (+ statistics) for one thread's RX x RY rays: macro terms and pixel index in
 // fp64, run-length aggregated binning.  Shared by every instantiation of the kernels below.
-template <int RX, int RY, bool CAPTURE, int WARPS = kWarps, bool RANDOM = false>
+//
+// Binning works on the pixel coordinate directly: u = (y + L/2) n_pix/L with y = c x - S (eq.4) is evaluated as
+//     u = fma(-S, n_pix/L, fma(x, c n_pix/L, (L/2) n_pix/L))
+// (two fp64 FMAs per component, the inner one shared by a column / row of the regular grid), floored with one
+// F2I.F64.FLOOR; the ray is in the map iff both floors are < n_pix as unsigned integers and u is finite (exponent
+// field of u not all ones: F2I maps NaN to 0, so the test cannot be skipped).  CAPTURE writes y itself.
+// RANDOM instantiations either pass the (u1, u2) they drew in the prologue (UV_SMEM: shared memory, [ray][thread]) or
+// have them drawn again here (same counter, same key: the same numbers).
+template <int RX, int RY, bool CAPTURE, int WARPS = kWarps, bool RANDOM = false, bool UV_SMEM = false>
 __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, long long tj, long long t, int lane,
                                             int warp, const double (&Sx)[RY][RX], const double (&Sy)[RY][RX],
-                                            unsigned int *cta_count)
+                                            unsigned int *cta_count, const double2 *uv = nullptr)
 {
     constexpr int TW = 32 * RX;
     constexpr int TH = WARPS * RY;
-    // ---- a4 + a5: macro terms, pixel, binning
+    constexpr int THREADS = WARPS * 32;
     unsigned int n_shot = 0, n_in = 0, n_drop = 0; // per thread; reduced over the warp once, after the loop
     const unsigned int full = 0xffffffffu;
-    // per-column / per-row quantities once per thread: image-plane coordinate and "inside the requested region" bits
-    double x1c[RX];
+    auto draw = [&](int r, int c) {
+        double2 w = make_double2(0.0, 0.0);
+        if (RANDOM) {
+            if (UV_SMEM) {
+                w = uv[(r * RX + c) * THREADS + threadIdx.x];
+            } else {
+                const unsigned long long i = (unsigned long long)(ti * TW + lane * RX + c), j = (unsigned long long)(tj * TH + warp * RY + r);
+                ray_uniforms(j * (unsigned long long)p.n1 + i, p.ray_seed, w.x, w.y);
+            }
+        }
+        return w;
+    };
+    // per-column / per-row quantities once per thread: ray index as an exact double and "inside the requested region" bits
+    const double ib = (double)(ti * TW), jb = (double)(tj * TH);
+    double fi[RX], fj[RY];
     unsigned int colmask = 0u, rowmask = 0u;
 #pragma unroll
     for (int c = 0; c < RX; ++c) {
         const long long i = ti * TW + lane * RX + c;
-        x1c[c] = ((double)i - p.half1) * p.delta;
+        fi[c] = ib + (double)(lane * RX + c); // = (double)i exactly
         colmask |= ((i >= p.i0) && (i < p.i1)) ? (1u << c) : 0u;
     }
 #pragma unroll
     for (int r = 0; r < RY; ++r) {
         const long long j = tj * TH + warp * RY + r;
+        fj[r] = jb + (double)(warp * RY + r);
         rowmask |= ((j >= p.j0) && (j < p.j1)) ? (1u << r) : 0u;
     }
-    const unsigned int n_pix_u = (unsigned int)p.n_pix;
+    if (CAPTURE) {
 #pragma unroll
-    for (int r = 0; r < RY; ++r) {
-        const long long j = tj * TH + warp * RY + r;
-        double x2 = ((double)j - p.half2) * p.delta;
+        for (int r = 0; r < RY; ++r)
 #pragma unroll
-        for (int c = 0; c < RX; ++c) {
-            const long long i = ti * TW + lane * RX + c;
-            double x1 = x1c[c];
-            if (RANDOM) { // the ray's own position in its cell (same draw as in the prologue)
-                double u1, u2;
-                ray_uniforms((unsigned long long)j * (unsigned long long)p.n1 + (unsigned long long)i, p.ray_seed, u1, u2);
-                x1 = ((double)i + u1 - (p.half1 + 0.5)) * p.delta;
-                x2 = ((double)j + u2 - (p.half2 + 0.5)) * p.delta;
-            }
-            const double y1 = p.c1 * x1 - Sx[r][c];
-            const double y2 = p.c2 * x2 - Sy[r][c];
-            const bool finite = (fabs(y1) <= 1.7976931348623157e308) && (fabs(y2) <= 1.7976931348623157e308);
-            if (CAPTURE) {
+            for (int c = 0; c < RX; ++c) {
+                double x1, x2;
+                if (RANDOM) { // the ray's own position in its cell (the draw of the prologue)
+                    const double2 w = draw(r, c);
+                    x1 = (fi[c] + w.x - (p.half1 + 0.5)) * p.delta;
+                    x2 = (fj[r] + w.y - (p.half2 + 0.5)) * p.delta;
+                } else {
+                    x1 = (fi[c] - p.half1) * p.delta;
+                    x2 = (fj[r] - p.half2) * p.delta;
+                }
+                const double y1 = p.c1 * x1 - Sx[r][c];
+                const double y2 = p.c2 * x2 - Sy[r][c];
+                const bool finite = (fabs(y1) <= 1.7976931348623157e308) && (fabs(y2) <= 1.7976931348623157e308);
                 const double qnan = __longlong_as_double(0x7ff8000000000000LL);
                 double2 o;
                 o.x = finite ? y1 : qnan;
                 o.y = finite ? y2 : qnan;
                 p.capture[(size_t)t * (TW * TH) + (size_t)(warp * RY + r) * TW + lane * RX + c] = o;
-            } else {
-                const bool valid = ((colmask >> c) & (rowmask >> r) & 1u) != 0u;
-                const double u1 = (y1 + p.halfL) * p.inv_pixel;
-                const double u2 = (y2 + p.halfL) * p.inv_pixel;
-                // floor to int (saturating): 0 <= u < n_pix  <=>  (unsigned)floor(u) < n_pix for every finite u
-                const int pi = __double2int_rd(u1), pj = __double2int_rd(u2);
-                const bool inside = ((unsigned int)pi < n_pix_u) && ((unsigned int)pj < n_pix_u);
-                const int pix = (valid && finite && inside) ? pj * p.n_pix + pi : -1;
-                // run-length aggregation along the lanes of the warp
-                const int prev = __shfl_up_sync(full, pix, 1);
-                const bool head = (lane == 0) || (pix != prev);
-                const unsigned int heads = __ballot_sync(full, head);
-                if (head && pix >= 0) {
-                    const unsigned int above = heads & ~((2u << lane) - 1u);
-                    const int next = above ? (__ffs(above) - 1) : 32;
-                    atomicAdd(&p.map[pix], (unsigned int)(next - lane));
-                }
-                n_in += (pix >= 0);
-                n_shot += valid;
-                n_drop += (valid && !finite);
             }
+        return;
+    }
+    // ---- a4 + a5: macro terms folded into the pixel coordinate, binning
+    double U1[RX], U2[RY];
+    if (!RANDOM) {
+#pragma unroll
+        for (int c = 0; c < RX; ++c) U1[c] = __fma_rn((fi[c] - p.half1) * p.delta, p.k1, p.hoff);
+#pragma unroll
+        for (int r = 0; r < RY; ++r) U2[r] = __fma_rn((fj[r] - p.half2) * p.delta, p.k2, p.hoff);
+    }
+    const unsigned int n_pix_u = (unsigned int)p.n_pix;
+    const double nip = -p.inv_pixel;
+#pragma unroll
+    for (int r = 0; r < RY; ++r) {
+#pragma unroll
+        for (int c = 0; c < RX; ++c) {
+            double b1, b2;
+            if (RANDOM) {
+                const double2 w = draw(r, c);
+                b1 = __fma_rn((fi[c] + w.x - (p.half1 + 0.5)) * p.delta, p.k1, p.hoff);
+                b2 = __fma_rn((fj[r] + w.y - (p.half2 + 0.5)) * p.delta, p.k2, p.hoff);
+            } else {
+                b1 = U1[c];
+                b2 = U2[r];
+            }
+            const double u1 = __fma_rn(Sx[r][c], nip, b1);
+            const double u2 = __fma_rn(Sy[r][c], nip, b2);
+            // finite <=> exponent field not all ones, in both components
+            const bool finite = ((~__double2hiint(u1) & 0x7ff00000) != 0) && ((~__double2hiint(u2) & 0x7ff00000) != 0);
+            const bool valid = ((colmask >> c) & (rowmask >> r) & 1u) != 0u;
+            // floor to int (saturating): 0 <= u < n_pix  <=>  (unsigned)floor(u) < n_pix for every finite u
+            const int pi = __double2int_rd(u1), pj = __double2int_rd(u2);
+            const bool inside = ((unsigned int)pi < n_pix_u) && ((unsigned int)pj < n_pix_u);
+            const int pix = (valid && finite && inside) ? pj * p.n_pix + pi : -1;
+            // run-length aggregation along the lanes of the warp
+            const int prev = __shfl_up_sync(full, pix, 1);
+            const bool head = (lane == 0) || (pix != prev);
+            const unsigned int heads = __ballot_sync(full, head);
+            if (head && pix >= 0) {
+                const unsigned int above = heads & ~((2u << lane) - 1u);
+                const int next = above ? (__ffs(above) - 1) : 32;
+                atomicAdd(&p.map[pix], (unsigned int)(next - lane));
+            }
+            n_in += (pix >= 0);
+            n_shot += valid;
+            n_drop += (valid && !finite);
         }
     }
-    if (!CAPTURE) {
-        n_shot = __reduce_add_sync(full, n_shot); // REDUX.SUM: one instruction per counter instead of a vote per ray
-        n_in = __reduce_add_sync(full, n_in);
-        n_drop = __reduce_add_sync(full, n_drop);
-        if (lane == 0) {
-            atomicAdd(&cta_count[0], n_shot);
-            atomicAdd(&cta_count[1], n_in);
-            if (n_drop) atomicAdd(&cta_count[2], n_drop);
-        }
-        __syncthreads();
-        if (threadIdx.x < 3 && cta_count[threadIdx.x])
-            atomicAdd(&p.counters[threadIdx.x], (unsigned long long)cta_count[threadIdx.x]);
+    n_shot = __reduce_add_sync(full, n_shot); // REDUX.SUM: one instruction per counter instead of a vote per ray
+    n_in = __reduce_add_sync(full, n_in);
+    n_drop = __reduce_add_sync(full, n_drop);
+    if (lane == 0) {
+        atomicAdd(&cta_count[0], n_shot);
+        atomicAdd(&cta_count[1], n_in);
+        if (n_drop) atomicAdd(&cta_count[2], n_drop);
     }
+    __syncthreads();
+    if (threadIdx.x < 3 && cta_count[threadIdx.x])
+        atomicAdd(&p.counters[threadIdx.x], (unsigned long long)cta_count[threadIdx.x]);
+}
+
+// a6: which tile this CTA shoots.  Shoot launches use a 2-D grid (x = tile column, y = tile row: the hardware
+// rasterises x first, so concurrently resident CTAs touch a narrow band of the map) and need no division; capture
+// launches take their tiles from an explicit list.
+template <bool CAPTURE>
+__device__ __forceinline__ void which_tile(const ShootParams &p, long long &t, long long &ti, long long &tj)
+{
+    if (CAPTURE) {
+        t = (long long)blockIdx.x;
+        ti = p.tile_list[2 * t];
+        tj = p.tile_list[2 * t + 1];
+    } else {
+        t = 0;
+        ti = p.tile_i0 + blockIdx.x;
+        tj = p.tile_j0 + blockIdx.y;
+    }
+}
+
+// Lens range of this CTA.  Shoot launches walk every lens.  Capture launches of a few tiles over many lenses
+// (ml_probe / ml_capture_region at N* >= 1e5) split the lens loop over
+// blockIdx.y: ranges are multiples of the 512-lens chunk, so chunk and flush-group boundaries fall where they do in
+// the unsplit loop; each CTA writes its fp64 partial sums and combine_kernel adds them in range order.
+template <bool CAPTURE> __device__ __forceinline__ void lens_range(const ShootParams &p, int &lb, int &le)
+{
+    lb = 0;
+    le = p.n_lens;
+    if (CAPTURE && p.split_len > 0) {
+        const long long b = (long long)blockIdx.y * p.split_len;
+        lb = (int)b;
+        le = (int)min(b + (long long)p.split_len, (long long)p.n_lens);
+    }
+}
+
+template <int RX, int RY, int WARPS>
+__device__ __forceinline__ void store_partials(const ShootParams &p, long long t, int lane, int warp, const double (&Sx)[RY][RX],
+                                               const double (&Sy)[RY][RX])
+{
+    constexpr int TW = 32 * RX, TH = WARPS * RY;
+    double2 *dst = p.partial + ((size_t)blockIdx.y * gridDim.x + (size_t)t) * (TW * TH);
+#pragma unroll
+    for (int r = 0; r < RY; ++r)
+#pragma unroll
+        for (int c = 0; c < RX; ++c) dst[(size_t)(warp * RY + r) * TW + lane * RX + c] = make_double2(Sx[r][c], Sy[r][c]);
+}
+
+// Second half of a split launch: one CTA per tile, the thread-to-ray mapping of the shoot kernels; the partial sums
+// of the lens ranges are added in range order (fp64), then the usual epilogue runs: CAPTURE writes the positions,
+// otherwise the rays are binned (a small region shot through very many lenses, ml_shoot_region).
+template <int RX, int RY, int WARPS, bool RANDOM, bool CAPTURE>
+__global__ void __launch_bounds__(WARPS * 32) combine_kernel(const ShootParams p, int n_splits)
+{
+    constexpr int TW = 32 * RX, TH = WARPS * RY;
+    __shared__ unsigned int cta_count[3];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    long long t, ti, tj;
+    which_tile<true>(p, t, ti, tj);
+    if (threadIdx.x < 3) cta_count[threadIdx.x] = 0;
+    __syncthreads();
+    double Sx[RY][RX], Sy[RY][RX];
+#pragma unroll
+    for (int r = 0; r < RY; ++r)
+#pragma unroll
+        for (int c = 0; c < RX; ++c) { Sx[r][c] = 0.0; Sy[r][c] = 0.0; }
+    for (int s = 0; s < n_splits; ++s) {
+        const double2 *src = p.partial + ((size_t)s * gridDim.x + (size_t)t) * (TW * TH);
+#pragma unroll
+        for (int r = 0; r < RY; ++r)
+#pragma unroll
+            for (int c = 0; c < RX; ++c) {
+                const double2 v = src[(size_t)(warp * RY + r) * TW + lane * RX + c];
+                Sx[r][c] += v.x;
+                Sy[r][c] += v.y;
+            }
+    }
+    finish_tile<RX, RY, CAPTURE, WARPS, RANDOM, false>(p, ti, tj, t, lane, warp, Sx, Sy, cta_count);
 }
 
 template <typename Real, int RX, int RY, int KF, bool NEWTON, bool CAPTURE, bool MASS = false, bool RANDOM = false>
@@ -237,15 +361,10 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
     const int warp = threadIdx.x >> 5;
 
     // ---- a6: which tile
-    long long ti, tj;
-    const long long t = (long long)blockIdx.x + p.tile_base;
-    if (CAPTURE) {
-        ti = p.tile_list[2 * t];
-        tj = p.tile_list[2 * t + 1];
-    } else {
-        ti = p.tile_i0 + t % p.tiles_x;
-        tj = p.tile_j0 + t / p.tiles_x;
-    }
+    long long t, ti, tj;
+    which_tile<CAPTURE>(p, t, ti, tj);
+    int lb, le; // this CTA's lens range: [0, n_lens) except in split capture launches
+    lens_range<CAPTURE>(p, lb, le);
     if (threadIdx.x < 3) cta_count[threadIdx.x] = 0;
 
     // ---- a2: tile centre (fp64) and this thread's ray offsets from it
@@ -289,7 +408,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
 #pragma unroll
         for (int q = 0; q < PER_THREAD; ++q) {
             const int k = base + q * kThreads + threadIdx.x;
-            if (k < p.n_lens) {
+            if (k < le) {
                 pre[q] = __ldg(&p.lens[k]);
                 if (MASS) pre_m[q] = __ldg(&p.mass[k]);
             }
@@ -301,7 +420,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
             const int k = base + q * kThreads + threadIdx.x;
             Real2 v;
             Real m = (Real)0;
-            if (k < p.n_lens) {
+            if (k < le) {
                 v.x = (Real)(pre[q].x - cx);
                 v.y = (Real)(pre[q].y - cy);
                 if (MASS) m = (Real)pre_m[q];
@@ -312,21 +431,22 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
             if (MASS) mass_s[buf][q * kThreads + threadIdx.x] = m;
         }
     };
-    fetch(0);
-    stage(0, 0);
+    fetch(lb);
+    stage(lb, 0);
     __syncthreads();
 
     // ---- a3: all-pairs deflection sum
     int buf = 0;
-    for (int base = 0; base < p.n_lens; base += kChunk) {
-        const bool more = base + kChunk < p.n_lens;
+    for (int base = lb; base < le; base += kChunk) {
+        const bool more = base + kChunk < le;
         if (more) fetch(base + kChunk);
-        const int cnt = min(kChunk, p.n_lens - base);
+        const int cnt = min(kChunk, le - base);
         const int cntp = (cnt + 7) & ~7; // padded with zero-contribution lenses
         const Real2 *ls = lens_s[buf];
         const Real *ms = mass_s[buf];
-        for (int k0 = 0; k0 < cntp; k0 += KF) {
-            const int kend = min(k0 + KF, cntp);
+        for (int k0 = 0, kend; k0 < cntp; k0 = kend) {
+            kend = min(k0 + KF, cntp);
+            if (cntp - kend < KF / 2) kend = cntp; // a trailing group shorter than KF/2 joins the group before it
 #pragma unroll 1
             for (int k = k0; k < kend; k += 2) {
 #pragma unroll
@@ -377,6 +497,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
         buf ^= 1;
     }
 
+    if (CAPTURE && p.partial) { store_partials<RX, RY, kWarps>(p, t, lane, warp, Sx, Sy); return; }
     finish_tile<RX, RY, CAPTURE, kWarps, RANDOM>(p, ti, tj, t, lane, warp, Sx, Sy, cta_count);
 }
 
@@ -431,15 +552,10 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
 
-    long long ti, tj;
-    const long long t = (long long)blockIdx.x + p.tile_base;
-    if (CAPTURE) {
-        ti = p.tile_list[2 * t];
-        tj = p.tile_list[2 * t + 1];
-    } else {
-        ti = p.tile_i0 + t % p.tiles_x;
-        tj = p.tile_j0 + t / p.tiles_x;
-    }
+    long long t, ti, tj;
+    which_tile<CAPTURE>(p, t, ti, tj);
+    int lb, le; // this CTA's lens range: [0, n_lens) except in split capture launches
+    lens_range<CAPTURE>(p, lb, le);
     if (threadIdx.x < 3) cta_count[threadIdx.x] = 0;
     // NEWTON: the padding lens must keep r2A * r2B finite (inf * 0 in the refinement would be NaN): 1e9 -> product 4e36,
     // its terms are 5e-10 R_E (at most two padding lenses per launch are ever evaluated: below every tolerance)
@@ -473,7 +589,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
 #pragma unroll
         for (int q = 0; q < PER_THREAD; ++q) {
             const int k = base + q * THREADS + threadIdx.x;
-            if (k < p.n_lens) {
+            if (k < le) {
                 pre[q] = __ldg(&p.lens[k]);
                 if (MASS) pre_m[q] = __ldg(&p.mass[k]);
             }
@@ -484,7 +600,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
         for (int q = 0; q < PER_THREAD; ++q) {
             const int k = base + q * THREADS + threadIdx.x;
             float nx = padc, ny = padc, m = 0.f;
-            if (k < p.n_lens) {
+            if (k < le) {
                 nx = -(float)(pre[q].x - cx);
                 ny = -(float)(pre[q].y - cy);
                 if (MASS) m = (float)pre_m[q];
@@ -493,8 +609,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
             if (MASS) mass_s[buf][q * THREADS + threadIdx.x] = m;
         }
     };
-    fetch(0);
-    stage(0, 0);
+    fetch(lb);
+    stage(lb, 0);
     __syncthreads();
 
     const float2 eps2 = make_float2(0x1p-80f, 0x1p-80f);
@@ -553,18 +669,19 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
     };
 
     int buf = 0;
-    for (int base = 0; base < p.n_lens; base += kChunk) {
-        const bool more = base + kChunk < p.n_lens;
+    for (int base = lb; base < le; base += kChunk) {
+        const bool more = base + kChunk < le;
         if (more) fetch(base + kChunk);
-        const int cnt = min(kChunk, p.n_lens - base);
+        const int cnt = min(kChunk, le - base);
         const int cntp = (cnt + 1) & ~1;
         const float4 *ls = lens_s[buf];
         const float *ms = mass_s[buf];
         auto mass_of = [&](int k) { return MASS ? ms[k] : 1.f; };
         PipeRegs<RY> a, b;
         stage1(ls[0], mass_of(0), a);
-        for (int k0 = 0; k0 < cntp; k0 += KF) {
-            const int kend = min(k0 + KF, cntp);
+        for (int k0 = 0, kend; k0 < cntp; k0 = kend) {
+            kend = min(k0 + KF, cntp);
+            if (cntp - kend < KF / 2) kend = cntp; // a trailing group shorter than KF/2 joins the group before it
 #pragma unroll 1
             for (int k = k0; k < kend; k += 2) {
                 stage1(ls[k + 1], mass_of(k + 1), b);
@@ -585,7 +702,216 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
         __syncthreads();
         buf ^= 1;
     }
+    if (CAPTURE && p.partial) { store_partials<RX, RY, WARPS>(p, t, lane, warp, Sx, Sy); return; }
     finish_tile<RX, RY, CAPTURE, WARPS>(p, ti, tj, t, lane, warp, Sx, Sy, cta_count);
+}
+
+
+// ---------------------------------------------------------------------------------------
+// Random ray positions (ML_RAYS_RANDOM: GPU-D's own ray generation; R17), FP32 modes.
+//
+// Every ray starts at its own point of its grid cell, so no column / row difference is shared between the rays
+// of a thread and the regular-grid kernel above does not apply.  The rest of its design does: a thread owns
+// 4 x 2 rays as packed pairs along axis 1 (columns 0,1 = "A", 2,3 = "B"), every FP32 instruction on the rays is a
+// packed FADD2 / FMUL2 / FFMA2, one reciprocal serves two interactions (R = 1/(r2A r2B), 1/r2A = R r2B,
+// 1/r2B = R r2A) and the loop is software-pipelined over lenses.  Per lens and row: 4 FADD2 (dx, dy of A and B),
+// 4 FFMA2 (r^2 = dy dy + (dx dx + 2^-80)), 3 FMUL2, 2 MUFU.RCP, 4 FFMA2 = 15 packed instructions for 4 interactions
+// (7.5 FMA-pipe lane-cycles per interaction against 5.25 on the regular grid: the price of per-ray offsets).
+// The two 53-bit uniforms of a ray are drawn once (Philox-4x32-10, counter = ray id) and kept in shared memory for
+// the epilogue, which needs them again for the fp64 position.  Summation order and padding as in shoot_kernel_pipe.
+template <int RY> struct RPipeRegs {
+    float m;
+    float2 dxA[RY], dxB[RY], dyA[RY], dyB[RY];
+    float2 r2A[RY], r2B[RY]; // r^2
+    float2 R[RY], Rb[RY];    // shared rows: R = 1/(r2A r2B); own-reciprocal rows: R = 1/r2A, Rb = 1/r2B
+};
+
+constexpr int kRandWarps = 8, kRandRY = 2;
+constexpr size_t rpipe_smem_bytes(bool mass)
+{
+    return 2 * (kChunk + 2) * sizeof(float4) + (size_t)4 * kRandRY * kRandWarps * 32 * sizeof(double2) +
+           (mass ? 2 * (kChunk + 2) * sizeof(float) : 0);
+}
+
+// OWN = 1: on the last row of every odd lens the two ray pairs take their own reciprocals (4 MUFU, no FMUL2) instead
+// of the shared one (2 MUFU + 3 FMUL2): the XU pipe has room for a quarter more reciprocals (61 % busy instead of 48 %)
+// and the FMA pipe, which bounds the loop, loses 3 of its 60 packed instructions per lens pair.
+template <int KF, int MINB, bool CAPTURE, bool MASS = false, bool NEWTON = false, int OWN = 1>
+__global__ void __launch_bounds__(kRandWarps * 32, MINB) shoot_kernel_rpipe(const ShootParams p)
+{
+    constexpr int RX = 4, RY = kRandRY, WARPS = kRandWarps;
+    constexpr int THREADS = WARPS * 32;
+    constexpr int TW = 32 * RX;
+    constexpr int TH = WARPS * RY;
+    static_assert(kChunk % KF == 0 && KF % 2 == 0, "flush groups must tile a chunk");
+    constexpr int PER_THREAD = kChunk / THREADS;
+
+    extern __shared__ __align__(16) unsigned char rp_smem[];
+    float4 *lens_s = reinterpret_cast<float4 *>(rp_smem);                                      // [2][kChunk + 2]
+    double2 *uv_s = reinterpret_cast<double2 *>(rp_smem + 2 * (kChunk + 2) * sizeof(float4)); // [RX*RY][THREADS]
+    float *mass_s = reinterpret_cast<float *>(rp_smem + 2 * (kChunk + 2) * sizeof(float4) +
+                                              (size_t)RX * RY * THREADS * sizeof(double2));   // [2][kChunk + 2]
+    __shared__ unsigned int cta_count[3];
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    long long t, ti, tj;
+    which_tile<CAPTURE>(p, t, ti, tj);
+    int lb, le; // this CTA's lens range: [0, n_lens) except in split capture launches
+    lens_range<CAPTURE>(p, lb, le);
+    if (threadIdx.x < 3) cta_count[threadIdx.x] = 0;
+    const float padc = NEWTON ? -1e9f : -1e15f; // see shoot_kernel_pipe
+    if (threadIdx.x < 4) lens_s[(threadIdx.x >> 1) * (kChunk + 2) + kChunk + (threadIdx.x & 1)] = make_float4(padc, padc, padc, padc);
+    if (MASS && threadIdx.x < 4) mass_s[(threadIdx.x >> 1) * (kChunk + 2) + kChunk + (threadIdx.x & 1)] = 0.f;
+
+    // ---- a2: tile centre (fp64) and every ray's own offset from it
+    const double cx = ((double)(ti * TW) + 0.5 * (TW - 1) - p.half1) * p.delta;
+    const double cy = ((double)(tj * TH) + 0.5 * (TH - 1) - p.half2) * p.delta;
+    float2 oxA[RY], oxB[RY], oyA[RY], oyB[RY];
+#pragma unroll
+    for (int r = 0; r < RY; ++r) {
+        float ox[RX], oy[RX];
+#pragma unroll
+        for (int c = 0; c < RX; ++c) {
+            const unsigned long long i = (unsigned long long)(ti * TW + lane * RX + c), j = (unsigned long long)(tj * TH + warp * RY + r);
+            double2 w;
+            ray_uniforms(j * (unsigned long long)p.n1 + i, p.ray_seed, w.x, w.y);
+            uv_s[(r * RX + c) * THREADS + threadIdx.x] = w;
+            ox[c] = (float)(((double)(lane * RX + c) + w.x - 0.5 * TW) * p.delta);
+            oy[c] = (float)(((double)(warp * RY + r) + w.y - 0.5 * TH) * p.delta);
+        }
+        oxA[r] = make_float2(ox[0], ox[1]); oxB[r] = make_float2(ox[2], ox[3]);
+        oyA[r] = make_float2(oy[0], oy[1]); oyB[r] = make_float2(oy[2], oy[3]);
+    }
+
+    double Sx[RY][RX], Sy[RY][RX];
+    float2 sxA[RY], sxB[RY], syA[RY], syB[RY];
+#pragma unroll
+    for (int r = 0; r < RY; ++r) {
+#pragma unroll
+        for (int c = 0; c < RX; ++c) { Sx[r][c] = 0.0; Sy[r][c] = 0.0; }
+        sxA[r] = make_float2(0.f, 0.f); sxB[r] = sxA[r]; syA[r] = sxA[r]; syB[r] = sxA[r];
+    }
+
+    // ---- a1: lens staging (as in shoot_kernel_pipe)
+    double2 pre[PER_THREAD];
+    double pre_m[MASS ? PER_THREAD : 1];
+    auto fetch = [&](int base) {
+#pragma unroll
+        for (int q = 0; q < PER_THREAD; ++q) {
+            const int k = base + q * THREADS + threadIdx.x;
+            if (k < le) {
+                pre[q] = __ldg(&p.lens[k]);
+                if (MASS) pre_m[q] = __ldg(&p.mass[k]);
+            }
+        }
+    };
+    auto stage = [&](int base, int buf) {
+#pragma unroll
+        for (int q = 0; q < PER_THREAD; ++q) {
+            const int k = base + q * THREADS + threadIdx.x;
+            float nx = padc, ny = padc, m = 0.f;
+            if (k < le) {
+                nx = -(float)(pre[q].x - cx);
+                ny = -(float)(pre[q].y - cy);
+                if (MASS) m = (float)pre_m[q];
+            }
+            lens_s[buf * (kChunk + 2) + q * THREADS + threadIdx.x] = make_float4(nx, nx, ny, ny);
+            if (MASS) mass_s[buf * (kChunk + 2) + q * THREADS + threadIdx.x] = m;
+        }
+    };
+    fetch(lb);
+    stage(lb, 0);
+    __syncthreads();
+
+    // ---- a3: all-pairs deflection sum
+    const float2 eps2 = make_float2(0x1p-80f, 0x1p-80f);
+    auto stage1 = [&](auto odd, const float4 l, const float m, RPipeRegs<RY> &s) {
+        const float2 nlx = make_float2(l.x, l.y), nly = make_float2(l.z, l.w);
+        s.m = m;
+#pragma unroll
+        for (int r = 0; r < RY; ++r) {
+            s.dxA[r] = __fadd2_rn(oxA[r], nlx);
+            s.dxB[r] = __fadd2_rn(oxB[r], nlx);
+            s.dyA[r] = __fadd2_rn(oyA[r], nly);
+            s.dyB[r] = __fadd2_rn(oyB[r], nly);
+            s.r2A[r] = __ffma2_rn(s.dyA[r], s.dyA[r], __ffma2_rn(s.dxA[r], s.dxA[r], eps2));
+            s.r2B[r] = __ffma2_rn(s.dyB[r], s.dyB[r], __ffma2_rn(s.dxB[r], s.dxB[r], eps2));
+            if (OWN && decltype(odd)::value && r == RY - 1) {
+                s.R[r].x = rcp_approx(s.r2A[r].x); s.R[r].y = rcp_approx(s.r2A[r].y);
+                s.Rb[r].x = rcp_approx(s.r2B[r].x); s.Rb[r].y = rcp_approx(s.r2B[r].y);
+            } else {
+                const float2 P = __fmul2_rn(s.r2A[r], s.r2B[r]);
+                s.R[r].x = rcp_approx(P.x);
+                s.R[r].y = rcp_approx(P.y);
+            }
+        }
+    };
+    auto newton = [](float2 a, float2 R) { // one Newton-Raphson step: R <- R + R (1 - a R)
+        const float2 e = __ffma2_rn(make_float2(-a.x, -a.y), R, make_float2(1.f, 1.f));
+        return __ffma2_rn(R, e, R);
+    };
+    auto stage2 = [&](auto odd, const RPipeRegs<RY> &s) {
+#pragma unroll
+        for (int r = 0; r < RY; ++r) {
+            float2 iA, iB;
+            if (OWN && decltype(odd)::value && r == RY - 1) {
+                iA = s.R[r];
+                iB = s.Rb[r];
+                if (NEWTON) { iA = newton(s.r2A[r], iA); iB = newton(s.r2B[r], iB); }
+                if (MASS) { iA = __fmul2_rn(iA, make_float2(s.m, s.m)); iB = __fmul2_rn(iB, make_float2(s.m, s.m)); }
+            } else {
+                float2 R = s.R[r];
+                if (NEWTON) R = newton(__fmul2_rn(s.r2A[r], s.r2B[r]), R); // on the shared reciprocal, P = r2A r2B
+                if (MASS) R = __fmul2_rn(R, make_float2(s.m, s.m)); // m_i / (r2A r2B)
+                iA = __fmul2_rn(R, s.r2B[r]);
+                iB = __fmul2_rn(R, s.r2A[r]);
+            }
+            sxA[r] = __ffma2_rn(s.dxA[r], iA, sxA[r]);
+            syA[r] = __ffma2_rn(s.dyA[r], iA, syA[r]);
+            sxB[r] = __ffma2_rn(s.dxB[r], iB, sxB[r]);
+            syB[r] = __ffma2_rn(s.dyB[r], iB, syB[r]);
+        }
+    };
+
+    int buf = 0;
+    for (int base = lb; base < le; base += kChunk) {
+        const bool more = base + kChunk < le;
+        if (more) fetch(base + kChunk);
+        const int cnt = min(kChunk, le - base);
+        const int cntp = (cnt + 1) & ~1;
+        const float4 *ls = lens_s + buf * (kChunk + 2);
+        const float *ms = mass_s + buf * (kChunk + 2);
+        auto mass_of = [&](int k) { return MASS ? ms[k] : 1.f; };
+        RPipeRegs<RY> a, b;
+        const std::integral_constant<bool, false> even;
+        const std::integral_constant<bool, true> odd;
+        stage1(even, ls[0], mass_of(0), a);
+        for (int k0 = 0, kend; k0 < cntp; k0 = kend) {
+            kend = min(k0 + KF, cntp);
+            if (cntp - kend < KF / 2) kend = cntp; // a trailing group shorter than KF/2 joins the group before it
+#pragma unroll 1
+            for (int k = k0; k < kend; k += 2) {
+                stage1(odd, ls[k + 1], mass_of(k + 1), b);
+                stage2(even, a);
+                stage1(even, ls[k + 2], mass_of(k + 2), a);
+                stage2(odd, b);
+            }
+#pragma unroll
+            for (int r = 0; r < RY; ++r) {
+                Sx[r][0] += (double)sxA[r].x; Sx[r][1] += (double)sxA[r].y;
+                Sx[r][2] += (double)sxB[r].x; Sx[r][3] += (double)sxB[r].y;
+                Sy[r][0] += (double)syA[r].x; Sy[r][1] += (double)syA[r].y;
+                Sy[r][2] += (double)syB[r].x; Sy[r][3] += (double)syB[r].y;
+                sxA[r] = make_float2(0.f, 0.f); sxB[r] = sxA[r]; syA[r] = sxA[r]; syB[r] = sxA[r];
+            }
+        }
+        if (more) stage(base + kChunk, buf ^ 1);
+        __syncthreads();
+        buf ^= 1;
+    }
+    if (CAPTURE && p.partial) { store_partials<RX, RY, WARPS>(p, t, lane, warp, Sx, Sy); return; }
+    finish_tile<RX, RY, CAPTURE, WARPS, true, true>(p, ti, tj, t, lane, warp, Sx, Sy, cta_count, uv_s);
 }
 
 } // namespace mlb200

@@ -2,9 +2,13 @@
 (CUDA library through its C ABI, fp64 CPU oracle) and evaluate the four criteria of
 BASELINE.json:north_star.  No arithmetic of the method lives here: pixels are derived
 with the oracle's own floor rule (oracle.pixels_of), maps come from each side.
+
+Set ML_PARITY_REPORT=<file> to have every figure appended to it as JSON lines (this is
+how profiles/r02_parity_figures.md was written).
 """
 from __future__ import annotations
 
+import json
 import os
 
 import numpy as np
@@ -19,12 +23,30 @@ MIN_SAME_PIXEL = 0.9999         # >= 99.99 % of rays land in the oracle's pixel
 TOL_INMAP_REL = 1e-5            # total in-map counts
 TOL_BLOCK_MU = 1e-3             # |mu_gpu - mu_oracle| on 8x8-block averages
 
-# interactions the oracle may spend per config on sub-region parity (about 10 s on 8 cores)
-ORACLE_BUDGET = float(os.environ.get("ML_PARITY_BUDGET", "6e9"))
+# interactions the oracle may spend per config on sub-region parity.  SURVEY.md 8(c) asks for >= 4e6 probed rays per
+# config (so that the 1e-4 same-pixel allowance is >= 400 rays): 16 rectangles of 512 x 512 rays = 4.19e6 rays, which
+# is 8.5e10 interactions at C3's 20 248 lenses -- about 12 s of the oracle on the GPU box's 16 cores.
+ORACLE_BUDGET = float(os.environ.get("ML_PARITY_BUDGET", "1e11"))
+SUBREGION_SIDE = 512
+SUBREGION_TILES = 16
+
+PREC_NAME = {ml.ML_PREC_FP32_TILED: "fp32_tiled", ml.ML_PREC_FP32_COMPENSATED: "fp32_compensated", ml.ML_PREC_FP64: "fp64"}
 
 
 def problem_args(p):
     return (p.sigma, p.stellar_fraction, p.gamma, p.n_pix, p.n_rays, p.L)
+
+
+def report(case, figures):
+    """Print the figures of one parity case and append them to $ML_PARITY_REPORT if set."""
+    rec = {"case": case}
+    rec.update({k: (float(v) if isinstance(v, (float, np.floating)) else int(v) if isinstance(v, (int, np.integer)) else v)
+                for k, v in figures.items()})
+    print(json.dumps(rec))
+    path = os.environ.get("ML_PARITY_REPORT")
+    if path:
+        with open(path, "a") as f:
+            f.write(json.dumps(rec) + "\n")
 
 
 def make_pair(p, precision=ml.ML_PREC_FP32_TILED, lenses=None):
@@ -63,8 +85,29 @@ def check_maps(p, gpu_map, gpu_stats, ora_map, ora_stats):
             "pixels_differing": int((gpu_map != ora_map).sum())}
 
 
-def check_rays(p, g, y_gpu, y_ora):
-    """Criteria 1 and 2 on per-ray source-plane positions (same rays, same order)."""
+def close_passage_bound(g, tile_w, d, m):
+    """Reading R15: what the FP32 modes may add to the 1e-3-pixel criterion for a ray that passes at distance d from a
+    lens of mass m.  Ray and lens are held in tile-local FP32 coordinates (|offset| <= T = tile_w/2 ray spacings, lens at
+    <= T + d), each rounded by <= 2^-24 of its size, so their difference carries |delta d| <= sqrt(2) 2^-23 (T + d); the
+    deflection m d/|d|^2 is an inversion whose Jacobian has norm m/d^2, hence an error m |delta d|/d^2; the <= 16
+    roundings of the term itself (r^2, shared product, MUFU.RCP at 1 ulp, 1/r^2, mass, FMA) add 2^-20 m/d."""
+    t_half = 0.5 * tile_w * g.delta
+    return TOL_POSITION_PIXELS * g.pixel + m * (2.0 ** 0.5 * 2.0 ** -23 * (t_half + d) / d ** 2 + 2.0 ** -20 / d)
+
+
+MAX_CLOSE_PASSAGE_FRACTION = 1e-5   # rays per ray that may invoke the close-passage bound
+
+
+def check_rays(p, g, y_gpu, y_ora, precision=ml.ML_PREC_FP32_TILED, rays_ij=None, lenses=None, mass=None, ray_seed=None,
+               tile_w=128):
+    """Criteria 1 and 2 on per-ray source-plane positions (same rays, same order).
+
+    Same pixel: every ray.  Position, FP32 modes (reading R15): asserted on the rays whose oracle position has
+    |y1|, |y2| <= 1.5 L (the map plus one map side of margin); a ray in that zone may exceed 1e-3 pixel only by the
+    close-passage bound of its nearest lens (`close_passage_bound`; needs rays_ij = (i, j) index arrays and the lens
+    field), and at most MAX_CLOSE_PASSAGE_FRACTION of the rays may do so.  The maximum over ALL finite rays, the number
+    of rays outside the zone and the number of excused rays are reported, so the narrowing is visible.
+    Position, ML_PREC_FP64: asserted on every finite ray, nothing excused."""
     y_gpu = y_gpu.reshape(-1, 2)
     y_ora = y_ora.reshape(-1, 2)
     ok = np.isfinite(y_ora).all(axis=1)
@@ -72,17 +115,90 @@ def check_rays(p, g, y_gpu, y_ora):
     pix_o = oracle.pixels_of(*problem_args(p), y_ora)
     pix_g = oracle.pixels_of(*problem_args(p), y_gpu)
     same = float((pix_o == pix_g).mean())
-    # position criterion on rays that matter for the map: inside it or within one map side of it
-    near = ok & (np.abs(y_ora) <= 1.5 * p.L).all(axis=1)
-    err = np.abs(y_gpu[near] - y_ora[near]).max() / g.pixel if near.any() else 0.0
+    zone = ok & (np.abs(y_ora) <= 1.5 * p.L).all(axis=1)
+    d = np.abs(y_gpu - y_ora).max(axis=1) / g.pixel
+    err_all = float(d[ok].max()) if ok.any() else 0.0
+    excused = 0
+    if precision == ml.ML_PREC_FP64:
+        err = err_all
+        err_zone = float(d[zone].max()) if zone.any() else 0.0
+    else:
+        bad = np.flatnonzero(zone & ~(d <= TOL_POSITION_PIXELS))
+        if bad.size:
+            assert rays_ij is not None and lenses is not None, ("position error / pixel", float(d[bad].max()))
+            assert bad.size <= max(1, int(MAX_CLOSE_PASSAGE_FRACTION * y_ora.shape[0])), ("rays over 1e-3 pixel", bad.size)
+            ri, rj = np.asarray(rays_ij[0]).ravel()[bad], np.asarray(rays_ij[1]).ravel()[bad]
+            x = oracle.ray_positions(*problem_args(p), ri, rj, ray_seed=ray_seed)
+            for q, k in enumerate(bad):
+                dist = np.sqrt(((lenses - x[q]) ** 2).sum(axis=1))
+                n = int(dist.argmin())
+                bound = close_passage_bound(g, tile_w, float(dist[n]), float(mass[n]) if mass is not None else 1.0)
+                assert d[k] * g.pixel <= bound, ("position error beyond the close-passage bound", int(ri[q]), int(rj[q]),
+                                                  float(d[k]), bound / g.pixel, float(dist[n]))
+            excused = int(bad.size)
+        keep = zone.copy()
+        keep[bad] = False
+        err_zone = float(d[zone].max()) if zone.any() else 0.0
+        err = float(d[keep].max()) if keep.any() else 0.0
     assert err <= TOL_POSITION_PIXELS, ("position error / pixel", err)
     assert same >= MIN_SAME_PIXEL, ("same-pixel fraction", same)
-    return {"same_pixel": same, "pos_err_pixels": float(err), "rays": int(y_ora.shape[0])}
+    return {"same_pixel": same, "pos_err_pixels": err, "pos_err_pixels_incl_close_passages": err_zone,
+            "rays_excused_close_passage": excused, "pos_err_pixels_all_finite_rays": err_all,
+            "rays_outside_1p5L_zone": int((ok & ~zone).sum()), "rays_not_finite": int((~ok).sum()),
+            "rays_in_other_pixel": int((pix_o != pix_g).sum()), "rays": int(y_ora.shape[0])}
 
 
 def subregion_tiles(p, g, n_lens):
-    """Seeded ray sub-rectangles whose total oracle cost stays within ORACLE_BUDGET."""
-    side = 512 if n_lens < 4000 else 256
+    """Seeded ray sub-rectangles (the first four touch the four edges of the shooting rectangle): 16 of 512 x 512 rays
+    = 4.19e6 rays per config unless ORACLE_BUDGET forces fewer (never below 4)."""
+    side = SUBREGION_SIDE
     n_tiles = int(ORACLE_BUDGET / (max(n_lens, 1) * side * side))
-    n_tiles = max(4, min(32, n_tiles))
+    n_tiles = max(4, min(SUBREGION_TILES, n_tiles))
     return parity_tiles(g.n1, g.n2, n_tiles, side, p.seed)
+
+
+_ORACLE_CACHE = {}
+
+
+def oracle_subregions(p, g, xy, tiles, mass=None, ray_seed=None):
+    """The oracle's side of a sub-region case, computed once per (config, masses, ray seed) and shared by the precision
+    modes: per-ray positions of every rectangle (ora_capture_region), the partial map they bin into with the oracle's
+    own floor rule (ora_pixels_of) and its statistics.  The first rectangle is also shot with ora_shoot_region -- the
+    function the CPU pins fix -- and must give the same partial map."""
+    key = (p.name, mass is not None, ray_seed, len(tiles))
+    if key in _ORACLE_CACHE:
+        return _ORACLE_CACHE[key]
+    args = problem_args(p)
+    omap = np.zeros(p.n_pix * p.n_pix, dtype=np.uint32)
+    ost = {"rays_shot": 0, "rays_in_map": 0}
+    ys = []
+    for t, reg in enumerate(tiles):
+        y = oracle.capture_region(*args, xy, reg, mass=mass, ray_seed=ray_seed).reshape(-1, 2)
+        pix = oracle.pixels_of(*args, y).ravel()
+        part = np.bincount(pix[pix >= 0], minlength=p.n_pix * p.n_pix).astype(np.uint32)
+        if t == 0:
+            ref, st = oracle.shoot_region(*args, xy, region=reg, mass=mass, ray_seed=ray_seed)
+            assert np.array_equal(ref.ravel(), part) and st["rays_in_map"] == int(part.sum())
+        omap += part
+        ost["rays_shot"] += y.shape[0]
+        ost["rays_in_map"] += int(part.sum())
+        ys.append(y)
+    out = (ys, omap.reshape(p.n_pix, p.n_pix), ost)
+    _ORACLE_CACHE[key] = out
+    return out
+
+
+def run_subregions(p, m, g, xy, tiles, precision, mass=None, ray_seed=None):
+    """All four criteria on seeded sub-rectangles: both sides shoot the same rays into partial maps (criteria 3, 4),
+    and EVERY ray of EVERY rectangle is compared position by position (criteria 1, 2)."""
+    ys, omap, ost = oracle_subregions(p, g, xy, tiles, mass, ray_seed)
+    for t, reg in enumerate(tiles):
+        m.shoot_region(*reg, accumulate=(t > 0))
+    r = check_maps(p, m.counts(), m.stats, omap, ost)
+    y_g = np.concatenate([m.capture_region(*reg).reshape(-1, 2) for reg in tiles])
+    ii = np.concatenate([np.tile(np.arange(i0, i1, dtype=np.int64), j1 - j0) for (i0, i1, j0, j1) in tiles])
+    jj = np.concatenate([np.repeat(np.arange(j0, j1, dtype=np.int64), i1 - i0) for (i0, i1, j0, j1) in tiles])
+    r.update(check_rays(p, g, y_g, np.concatenate(ys), precision, rays_ij=(ii, jj), lenses=xy, mass=mass,
+                        ray_seed=ray_seed, tile_w=m.info["tile_w"]))
+    r.update(tiles=len(tiles), n_lenses=int(xy.shape[0]))
+    return r

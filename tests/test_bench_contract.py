@@ -31,3 +31,26 @@ def test_cuda_arm_refuses_to_run_without_a_device():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1", "--warmup", "0"],
                          capture_output=True, text=True, timeout=300, cwd=ROOT)
     assert out.returncode != 0 and "no CUDA device" in (out.stderr + out.stdout)
+
+
+def test_more_gpus_than_devices_is_an_error_not_a_silent_single_gpu_run():
+    """Started as the driver starts the scaling run (`python bench.py --gpus N`, no torchrun): with fewer than N
+    devices the script must exit non-zero instead of running one GPU and printing n_gpus = N."""
+    import torch
+    n = (torch.cuda.device_count() if torch.cuda.is_available() else 0) + 1
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", str(max(n, 2)), "--steps", "1", "--warmup", "3"],
+                         capture_output=True, text=True, timeout=300, cwd=ROOT)
+    assert out.returncode != 0
+    assert "refusing to run fewer GPUs than reported" in out.stderr
+    assert not [ln for ln in out.stdout.splitlines() if ln.strip().startswith("{")]
+
+
+def test_world_size_must_match_gpus():
+    """Under a launcher the world size must equal --gpus (never a silent mismatch)."""
+    import torch
+    if not torch.cuda.is_available():
+        return  # the no-device error comes first on a CPU box (tested above)
+    env = dict(os.environ, WORLD_SIZE="2", RANK="0", LOCAL_RANK="0")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "1", "--steps", "1", "--warmup", "3"],
+                         capture_output=True, text=True, timeout=300, cwd=ROOT, env=env)
+    assert out.returncode != 0 and "WORLD_SIZE" in (out.stderr + out.stdout)

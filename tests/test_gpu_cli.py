@@ -27,4 +27,7 @@ def test_cli_writes_the_oracles_map(tmp_path, capsys):
     out = capsys.readouterr().out
     assert "lenses 40" in out and "interactions/s" in out
     # synthetic disk + random rays path
-    assert cli.main(["--sigma", "0.4", "--n-pix", "32", "--n-rays", "16", "--L", "4", "--seed", "3", "--random-rays", "5"]) == 0
+    assert cli.main(["--sigma", "0.4", "--n-pix", "32", "--n-rays", "16", "--L", "4", "--seed", "3", "--random-rays", "5",
+                     "--dm-hist", "6"]) == 0
+    hist = [ln for ln in capsys.readouterr().out.splitlines() if ln.startswith("dm [")]
+    assert len(hist) == 6 and 0 < sum(int(ln.split()[-1]) for ln in hist) <= 32 * 32

@@ -47,7 +47,7 @@ def test_single_lens_at_origin(precision):
         check_maps(p, m.counts(), m.stats, omap, ost)
         y_g = m.capture_region(0, g.n1, 0, g.n2)
         y_o = oracle.capture_region(*problem_args(p), xy, (0, g.n1, 0, g.n2))
-        check_rays(p, g, y_g, y_o)
+        check_rays(p, g, y_g, y_o, precision)
 
 
 @pytest.mark.parametrize("n", [1, 2, 7, 8, 9, 63, 64, 65, 511, 512, 513, 1025, 1536])
@@ -88,27 +88,14 @@ def test_lens_count_boundaries_in_the_other_kernel_instantiations(n, masses, ran
         y_g = m.capture_region(0, g.n1, 0, g.n2)
         y_o = oracle.capture_region(*problem_args(p), xy, (0, g.n1, 0, g.n2), mass=mass, ray_seed=seed)
         info = m.info
-    # This problem has coarse rays (delta = 0.021 R_E, tile half-width T = 64 delta = 1.3 R_E), so in the FP32 modes a ray
-    # that passes within d of a lens carries the rounding of its tile-local coordinates, 2^-23 T, as a relative error
-    # 2^-23 T / d of a deflection m / d: more than 1e-3 pixel for d < d_crit = sqrt(2^-23 T m / (1e-3 pixel)) (reading
-    # R15; the five BASELINE configs have T <= 0.13 R_E and such rays leave the map's neighbourhood).  Those rays, and
-    # only those, are excused from the position criterion here; the same-pixel criterion applies to every ray.
-    err = np.abs(y_g - y_o).max(axis=-1) / g.pixel
-    near = np.isfinite(y_o).all(axis=-1) & (np.abs(y_o) <= 1.5 * p.L).all(axis=-1)
-    bad = np.argwhere(near & ~(err <= 1e-3))
-    if precision == ml.ML_PREC_FP64:
-        assert bad.size == 0
-    else:
-        assert len(bad) <= 3
-        t_half = 0.5 * info["tile_w"] * g.delta
-        m_max = float(mass.max()) if masses else 1.0
-        d_crit = 2.0 * (2.0 ** -23 * t_half * m_max / (1e-3 * g.pixel)) ** 0.5
-        for jj, ii in bad:
-            x = oracle.ray_positions(*problem_args(p), [ii], [jj], ray_seed=seed)[0]
-            assert np.sqrt(((xy - x) ** 2).sum(axis=1)).min() < d_crit, (ii, jj, err[jj, ii])
-    keep = np.ones(err.shape, dtype=bool)
-    keep[tuple(bad.T)] = False
-    check_rays(p, g, y_g[keep], y_o[keep])
+    # This problem has coarse rays (delta = 0.021 R_E, tile half-width T = 64 delta = 1.3 R_E), so in the FP32 modes a
+    # handful of rays that pass close to a lens exceed 1e-3 pixel by the rounding of their tile-local coordinates: reading
+    # R15, parity_common.close_passage_bound.  check_rays excuses those rays, and only those, from the position criterion
+    # (each must stay inside the bound of its nearest lens; ML_PREC_FP64 excuses nothing); the same-pixel criterion
+    # applies to every ray.
+    jj, ii = np.meshgrid(np.arange(g.n2, dtype=np.int64), np.arange(g.n1, dtype=np.int64), indexing="ij")
+    r = check_rays(p, g, y_g, y_o, precision, rays_ij=(ii, jj), lenses=xy, mass=mass, ray_seed=seed, tile_w=info["tile_w"])
+    assert r["rays_excused_close_passage"] <= 3
 
 
 @pytest.mark.parametrize("precision", ALL)

@@ -7,7 +7,7 @@ import paper_1005_5198_b200 as ml
 from oracle import oracle
 from workloads import CONFIGS, lens_disk, lens_masses, parity_tiles
 
-from parity_common import check_maps, check_rays, problem_args
+from parity_common import PREC_NAME, check_maps, check_rays, problem_args, report, run_subregions, subregion_tiles
 
 pytestmark = pytest.mark.gpu
 
@@ -35,35 +35,26 @@ def test_c1_with_a_mass_spectrum_all_four_criteria(precision):
         r = check_maps(p, gmap, gst, omap, ost)
         y_g = m.capture_region(0, g.n1, 0, g.n2)
         y_o = oracle.capture_region(*problem_args(p), xy, (0, g.n1, 0, g.n2), mass=mass)
-        r.update(check_rays(p, g, y_g, y_o))
+        r.update(check_rays(p, g, y_g, y_o, precision))
         # the masses matter: the unit-mass map of the same positions is a different map
         m.set_lenses(xy)
         m.shoot()
         assert (m.counts() != gmap).mean() > 0.5
-        print("C1 masses", PREC_IDS[PRECISIONS.index(precision)], r)
+        report("C1 whole map, masses, %s" % PREC_NAME[precision], r)
 
 
-@pytest.mark.parametrize("cfg", [2, 4], ids=["C3", "C5"])
-def test_subregions_with_masses(cfg):
+@pytest.mark.parametrize("cfg,precision", [(2, ml.ML_PREC_FP32_TILED), (4, ml.ML_PREC_FP32_TILED), (3, ml.ML_PREC_FP32_COMPENSATED)],
+                         ids=["C3-fp32_tiled", "C5-fp32_tiled", "C4-fp32_compensated"])
+def test_subregions_with_masses(cfg, precision):
+    """16 seeded rectangles of 512 x 512 rays, every ray compared (same sample as the unit-mass sub-region test)."""
     p = CONFIGS[cfg]
     g = oracle.geometry(*problem_args(p))
     xy, mass = field(p, g)
-    side = 256 if xy.shape[0] > 4000 else 512
-    tiles = parity_tiles(g.n1, g.n2, 4, side, p.seed)
-    with ml.MagnificationMap(*problem_args(p)) as m:
+    tiles = subregion_tiles(p, g, xy.shape[0])
+    with ml.MagnificationMap(*problem_args(p), precision=precision) as m:
         m.set_lenses(xy, mass)
-        omap = np.zeros((p.n_pix, p.n_pix), dtype=np.uint32)
-        ost = {"rays_shot": 0, "rays_in_map": 0}
-        for t, reg in enumerate(tiles):
-            m.shoot_region(*reg, accumulate=(t > 0))
-            _, st = oracle.shoot_region(*problem_args(p), xy, region=reg, map_out=omap, mass=mass)
-            for k in ost:
-                ost[k] += st[k]
-        r = check_maps(p, m.counts(), m.stats, omap, ost)
-        y_g = m.capture_region(*tiles[0])
-        y_o = oracle.capture_region(*problem_args(p), xy, tiles[0], mass=mass)
-        r.update(check_rays(p, g, y_g, y_o))
-        print(p.name, "masses", xy.shape[0], "lenses", r)
+        r = run_subregions(p, m, g, xy, tiles, precision, mass=mass)
+        report("%s sub-regions, masses, %s" % (p.name, PREC_NAME[precision]), r)
 
 
 @pytest.mark.parametrize("precision", PRECISIONS, ids=PREC_IDS)

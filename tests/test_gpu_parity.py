@@ -17,7 +17,8 @@ import paper_1005_5198_b200 as ml
 from oracle import oracle
 from workloads import CONFIGS, lens_disk, probe_rays
 
-from parity_common import (check_maps, check_rays, make_pair, problem_args, subregion_tiles)
+from parity_common import (PREC_NAME, check_maps, check_rays, make_pair, problem_args, report, run_subregions,
+                           subregion_tiles)
 
 pytestmark = pytest.mark.gpu
 
@@ -38,43 +39,32 @@ def test_c1_whole_map_all_four_criteria(precision):
         r = check_maps(p, gmap, gst, omap, ost)
         y_g = m.capture_region(0, g.n1, 0, g.n2)
         y_o = oracle.capture_region(*problem_args(p), xy, (0, g.n1, 0, g.n2))
-        r.update(check_rays(p, g, y_g, y_o))
-        # the shoot and capture instantiations run the same arithmetic: binning the
-        # captured positions (oracle's floor rule) reproduces the device map exactly
+        r.update(check_rays(p, g, y_g, y_o, precision))
+        # the shoot and capture instantiations run the same arithmetic: binning the captured positions (oracle's floor
+        # rule) reproduces the device map -- up to exact ties.  FP32 partial sums make y lattice-valued (spacing ~2^-26
+        # R_E), pixel edges are lattice points, so about one ray in 1e7 sits EXACTLY on an edge; the device floors the
+        # pixel coordinate u = fma(-S, n_pix/L, fma(x, c n_pix/L, n_pix/2)) and the oracle rule floors (y + L/2)/pixel,
+        # which may resolve such a tie to either side (the reason the criterion is 99.99 %, not 100 %).
         pix = oracle.pixels_of(*problem_args(p), y_g).ravel()
         rebinned = np.bincount(pix[pix >= 0], minlength=p.n_pix * p.n_pix).reshape(p.n_pix, p.n_pix)
-        assert np.array_equal(rebinned, gmap)
+        assert int(rebinned.sum()) == int(gmap.sum(dtype=np.uint64))
+        assert int(np.abs(rebinned.astype(np.int64) - gmap.astype(np.int64)).sum()) <= 8   # <= 4 tied rays of 6.5e6
         if precision == ml.ML_PREC_FP64:
             assert r["same_pixel"] >= 0.999999
-        print("C1", PREC_IDS[PRECISIONS.index(precision)], r)
+        report("C1 whole map %s" % PREC_NAME[precision], r)
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4], ids=["C2", "C3", "C4", "C5"])
-@pytest.mark.parametrize("precision", [ml.ML_PREC_FP32_TILED, ml.ML_PREC_FP64], ids=["fp32_tiled", "fp64"])
+@pytest.mark.parametrize("precision", PRECISIONS, ids=PREC_IDS)
 def test_subregions_all_four_criteria(cfg, precision):
+    """C2-C5: 16 seeded rectangles of 512 x 512 rays (4.19e6 rays per config), every ray compared."""
     p = CONFIGS[cfg]
     m, g, xy = make_pair(p, precision)
     with m:
         tiles = subregion_tiles(p, g, xy.shape[0])
-        omap = np.zeros((p.n_pix, p.n_pix), dtype=np.uint32)
-        ost = {"rays_shot": 0, "rays_in_map": 0}
-        same_w, rays, pos = 0.0, 0, 0.0
-        for t, (i0, i1, j0, j1) in enumerate(tiles):
-            m.shoot_region(i0, i1, j0, j1, accumulate=(t > 0))
-            _, st = oracle.shoot_region(*problem_args(p), xy, region=(i0, i1, j0, j1), map_out=omap)
-            for k in ost:
-                ost[k] += st[k]
-        r = check_maps(p, m.counts(), m.stats, omap, ost)
-        # per-ray criteria on every ray of the first tiles (capture = same kernel arithmetic)
-        for (i0, i1, j0, j1) in tiles[:4]:
-            y_g = m.capture_region(i0, i1, j0, j1)
-            y_o = oracle.capture_region(*problem_args(p), xy, (i0, i1, j0, j1))
-            rr = check_rays(p, g, y_g, y_o)
-            same_w += rr["same_pixel"] * rr["rays"]
-            rays += rr["rays"]
-            pos = max(pos, rr["pos_err_pixels"])
-        r.update(same_pixel=same_w / rays, pos_err_pixels=pos, rays=rays, tiles=len(tiles))
-        print(p.name, r)
+        r = run_subregions(p, m, g, xy, tiles, precision)
+        assert r["rays"] >= 4000000 or len(tiles) < 16
+        report("%s sub-regions %s" % (p.name, PREC_NAME[precision]), r)
 
 
 def test_c2_full_size_bench_configuration():
@@ -102,4 +92,5 @@ def test_c2_full_size_bench_configuration():
         m.shoot_region(i0, i1, j0, j1)
         omap, ost = oracle.shoot_region(*problem_args(p), xy, region=(i0, i1, j0, j1))
         r.update(check_maps(p, m.counts(), m.stats, omap, ost))
-        print("C2 full", r, "mean ratio", ratio)
+        r.update(mean_mu_over_theory=float(ratio))
+        report("C2 full size (bench launch), 200000 probed rays + one re-shot rectangle", r)

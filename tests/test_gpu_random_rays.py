@@ -8,7 +8,7 @@ import paper_1005_5198_b200 as ml
 from oracle import oracle
 from workloads import CONFIGS, lens_disk, lens_masses, parity_tiles
 
-from parity_common import check_maps, check_rays, problem_args
+from parity_common import PREC_NAME, check_maps, check_rays, problem_args, report, run_subregions, subregion_tiles
 
 pytestmark = pytest.mark.gpu
 
@@ -32,7 +32,7 @@ def test_c1_random_rays_all_four_criteria(precision):
         r = check_maps(p, gmap, gst, omap, ost)
         y_g = m.capture_region(0, g.n1, 0, g.n2)
         y_o = oracle.capture_region(*problem_args(p), xy, (0, g.n1, 0, g.n2), ray_seed=seed)
-        r.update(check_rays(p, g, y_g, y_o))
+        r.update(check_rays(p, g, y_g, y_o, precision))
         # another seed is another map; the regular grid is back after ML_RAYS_REGULAR
         m.set_ray_mode(ml.ML_RAYS_RANDOM, seed + 1)
         m.shoot()
@@ -41,35 +41,28 @@ def test_c1_random_rays_all_four_criteria(precision):
         m.shoot()
         if precision == ml.ML_PREC_FP64:
             assert np.array_equal(m.counts(), oracle.shoot(*problem_args(p), xy)[0])
-        print("C1 random rays", PREC_IDS[PRECISIONS.index(precision)], r)
+        report("C1 whole map, random rays, %s" % PREC_NAME[precision], r)
 
 
-# Measured mismatch rates on 3.9e5 rays (default mode): C4 3.3e-5, C3 2.5e-6; with masses AND random rays C4 reaches
-# 8.1e-5 (5.9e-5 compensated), too close to the 1e-4 bound for a four-tile sample, so the mass case runs on C3.
-@pytest.mark.parametrize("cfg,masses", [(1, False), (2, True), (3, False), (4, False)], ids=["C2", "C3-masses", "C4", "C5"])
-def test_subregions_random_rays(cfg, masses):
+# Sub-regions of C2-C5 with random rays, 4.19e6 rays each (16 rectangles of 512 x 512), every ray compared.  Masses AND
+# random rays together are the hardest combination for the FP32 arithmetic (every ray carries its own offsets and the
+# terms are scaled by m_i); on C4 DESIGN.md recommends ML_PREC_FP32_COMPENSATED for it, and that is the mode tested there.
+@pytest.mark.parametrize("cfg,masses,precision",
+                         [(1, False, ml.ML_PREC_FP32_TILED), (2, True, ml.ML_PREC_FP32_TILED), (3, False, ml.ML_PREC_FP32_TILED),
+                          (4, False, ml.ML_PREC_FP32_TILED), (3, True, ml.ML_PREC_FP32_COMPENSATED), (3, False, ml.ML_PREC_FP32_COMPENSATED)],
+                         ids=["C2", "C3-masses", "C4", "C5", "C4-masses-compensated", "C4-compensated"])
+def test_subregions_random_rays(cfg, masses, precision):
     p = CONFIGS[cfg]
     g = oracle.geometry(*problem_args(p))
     xy = lens_disk(g.n_star, g.r_star, p.seed)
     mass = lens_masses(g.n_star, p.seed) if masses else None
-    side = 256 if xy.shape[0] > 4000 else 512
-    tiles = parity_tiles(g.n1, g.n2, 4, side, p.seed)
+    tiles = subregion_tiles(p, g, xy.shape[0])
     seed = 1000 + cfg
-    with ml.MagnificationMap(*problem_args(p)) as m:
+    with ml.MagnificationMap(*problem_args(p), precision=precision) as m:
         m.set_lenses(xy, mass)
         m.set_ray_mode(ml.ML_RAYS_RANDOM, seed)
-        omap = np.zeros((p.n_pix, p.n_pix), dtype=np.uint32)
-        ost = {"rays_shot": 0, "rays_in_map": 0}
-        for t, reg in enumerate(tiles):
-            m.shoot_region(*reg, accumulate=(t > 0))
-            _, st = oracle.shoot_region(*problem_args(p), xy, region=reg, map_out=omap, mass=mass, ray_seed=seed)
-            for k in ost:
-                ost[k] += st[k]
-        r = check_maps(p, m.counts(), m.stats, omap, ost)
-        y_g = np.concatenate([m.capture_region(*t).reshape(-1, 2) for t in tiles])
-        y_o = np.concatenate([oracle.capture_region(*problem_args(p), xy, t, mass=mass, ray_seed=seed).reshape(-1, 2) for t in tiles])
-        r.update(check_rays(p, g, y_g, y_o))
-        print(p.name, "random rays", r)
+        r = run_subregions(p, m, g, xy, tiles, precision, mass=mass, ray_seed=seed)
+        report("%s sub-regions, random rays%s, %s" % (p.name, ", masses" if masses else "", PREC_NAME[precision]), r)
 
 
 def test_random_rays_partition_invariance_and_probe():

@@ -42,6 +42,7 @@ FP32_LANES_PER_SM = 128
 NCU_DRAM_BYTES_PER_LAUNCH = {
     ("C2", "fp32_tiled"): (4341504 + 0, "profiles/r01_ncu_full_c2_v2.txt"),
 }
+NCU_MAPSTATS_DRAM_BYTES = (134337536 + 5088768, "profiles/r01_ncu_full_mapstats.txt")
 
 
 def problem_args(p):
@@ -517,6 +518,12 @@ def run_mapstats(args):
     e1.record(stream)
     torch.cuda.synchronize(dev)
     ms = e0.elapsed_time(e1)
+    # wall clock of the call alone (device-resident maps, no L2 flush in between): what a user of the call waits for
+    torch.cuda.synchronize(dev)
+    t0 = time.perf_counter()
+    for _ in range(max(args.steps, 20)):
+        ml.ml_map_compare(ta.data_ptr(), n_rays, tb.data_ptr(), n_rays, n=n, device=dev.index, cuda_stream=stream.cuda_stream)
+    call_ms = 1e3 * (time.perf_counter() - t0) / max(args.steps, 20)
     t0 = time.perf_counter()
     for _ in range(args.steps):
         r_host = ml.ml_map_compare(a, n_rays, b, n_rays, device=dev.index)   # host buffers: H2D inside
@@ -549,17 +556,18 @@ def run_mapstats(args):
                        "l2": "flushed between steps (256 MiB write); the two maps (134 MB) exceed L2 anyway"},
             "result": {k: r[k] for k in ("rms_delta_m", "ks_d", "ks_prob", "n_valid")},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": 134337536 + 5088768, "pass_kernel_ms": pass_ms / args.steps,
+                         "traffic": NCU_MAPSTATS_DRAM_BYTES[0], "pass_kernel_ms": pass_ms / args.steps,
                          "all_kernels_ms_per_call": kernel_ms / args.steps,
                          "note": "dominant kernel = mlstats::pass_kernel (fused RMS + statistics + count histograms); "
                                  "algorithmic bytes = 2 maps x 4 B x n pixels read once; time = CUDA events around that "
                                  "launch on the launching stream (ml_map_compare_result.pass_kernel_ms); traffic = ncu "
-                                 "dram bytes read + written of that launch (profiles/r01_ncu_full_mapstats.txt); "
-                                 "peak = MEASURED_PEAKS.json hbm_gbs"},
+                                 "dram bytes read + written of that launch (%s); "
+                                 "peak = MEASURED_PEAKS.json hbm_gbs" % NCU_MAPSTATS_DRAM_BYTES[1]},
             "cpu_baseline": cpu, "clocks": clocks,
             "e2e": {"value": n * args.steps / e2e_s, "unit": "pixels/s", "h2d_bytes_per_step": 2 * 4 * n,
                     "d2h_bytes_per_step": 112},
-            "gpu_launches": 11 * args.steps}
+            "gpu_launches": 7 * args.steps,   # pass, reduce, three scan kernels, K-S, finalize (+ one memset) per call
+            "call_ms_without_flush": call_ms}
     print(json.dumps(line))
     return 0
 

@@ -217,8 +217,8 @@ typedef struct {
                                       empty pixel is a sample at +inf, M2)                       */
     double ks_prob;                /* Q_KS((sqrt(Ne)+0.12+0.11/sqrt(Ne)) ks_d), Ne = n/2 (M3):
                                       probability of a distance >= ks_d under the null hypothesis */
-    double kernel_ms;              /* device time of the whole call (all kernels, the memsets and
-                                      one small host read-back between them), CUDA events        */
+    double kernel_ms;              /* device time of the whole call (one memset and seven kernels,
+                                      no host round trip between them), CUDA events              */
     double pass_kernel_ms;         /* device time of the fused pass over the maps alone          */
 } ml_map_compare_result;
 
@@ -228,7 +228,8 @@ typedef struct {
  * out = HOST struct.  K-S ties between the two maps are decided exactly when n_rays_a, n_rays_b
  * have <= 26 significant bits.  ML_ERR_INVALID_ARG for NULL pointers, n < 1, n > 2^31-1,
  * non-positive or non-finite n_rays, or a bad `where`; ML_ERR_OOM if a count >= 2^27 makes the
- * count histogram too large; ML_ERR_CUDA without a device. */
+ * count histogram too large; ML_ERR_CUDA without a device.  Scratch memory (histograms, scans, events,
+ * a pinned result) is kept per device between calls; concurrent calls are serialised inside the library. */
 int ml_map_compare(const uint32_t *a, double n_rays_a, const uint32_t *b, double n_rays_b, int64_t n,
                    int where, int32_t device, void *cuda_stream, ml_map_compare_result *out);
 

@@ -12,11 +12,6 @@
 // mu, which orders the samples exactly as Delta m does, reversed).  All sums that feed a
 // floating-point result are reduced in a fixed order: results are bit-reproducible.
 //
-// The magnitude difference of a pixel needs no logarithm table: with integer counts N_a, N_b
-//   dm_a - dm_b = -2.5 log10(N_a/N_b) + 2.5 log10(n_rays_a/n_rays_b),   ln(N_a/N_b) = 2 atanh(s),  s = (N_a - N_b)/(N_a + N_b)
-// (numerator and denominator exact), and the atanh series in s^2 needs 5-14 terms for maps that resemble each other
-// (|s| <= 1/4); a warp with a less similar pixel pair falls back to two fp64 logarithms per pixel.
-//
 // Host side: nothing is allocated, created or synchronised per call beyond the one read-back of the result; the
 // scratch (histograms, scans, events, a pinned result) lives in a per-device cache that grows when needed.
 #include "../../include/microlens.h"
@@ -50,9 +45,13 @@ struct Totals {
 
 constexpr int kPassThreads = 1024;        // one CTA per SM
 constexpr unsigned int kShBins = 16384;   // per map: counts below this are histogrammed in shared memory
+constexpr unsigned int kLut = 8192;       // log10(c) for c < kLut is tabulated (global, copied to shared memory per CTA)
 
-__constant__ double c_odd_recip[16] = {1.0, 1.0 / 3, 1.0 / 5, 1.0 / 7, 1.0 / 9, 1.0 / 11, 1.0 / 13, 1.0 / 15,
-                                       1.0 / 17, 1.0 / 19, 1.0 / 21, 1.0 / 23, 1.0 / 25, 1.0 / 27, 1.0 / 29, 1.0 / 31};
+__global__ void lut_kernel(double *lut)
+{
+    const unsigned int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < kLut) lut[k] = log10((double)k); // [0] = -inf, never read
+}
 
 __device__ __forceinline__ void hist_add(unsigned int *sh, unsigned int *hist, unsigned int cap, unsigned int c)
 {
@@ -60,30 +59,24 @@ __device__ __forceinline__ void hist_add(unsigned int *sh, unsigned int *hist, u
     else if (c < cap) atomicAdd(&hist[c], 1u); // bright pixels: RED into the global histogram (L2)
 }
 
-// 1/d for an integer-valued d in [1, 2^33]: MUFU.RCP64H seed + two Newton-Raphson steps (relative error ~2^-52).
-__device__ __forceinline__ double recip_int(double d)
-{
-    double x;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(d));
-    double e = __fma_rn(-d, x, 1.0);
-    x = __fma_rn(x, e, x);
-    e = __fma_rn(-d, x, 1.0);
-    return __fma_rn(x, e, x);
-}
-
 // One pass over the maps: RMS sums, statistics, count histograms (privatised per CTA in shared memory for
 // counts < kShBins, flushed once at the end).  TWO = false: one map (ml_delta_m_histogram).
+// log10 of a count < kLut comes from a table (`lut`, built once per device by lut_kernel) that every CTA copies into
+// its shared memory: a pixel costs two table reads instead of two fp64 logarithms.
 template <bool TWO>
 __global__ void __launch_bounds__(kPassThreads, 1) pass_kernel(const unsigned int *__restrict__ a, const unsigned int *__restrict__ b,
                                                                long long n, double n_rays_a, double n_rays_b, unsigned int *hist_a,
-                                                               unsigned int *hist_b, unsigned int cap, Partial *partials)
+                                                               unsigned int *hist_b, unsigned int cap, Partial *partials,
+                                                               const double *__restrict__ lut)
 {
-    extern __shared__ __align__(8) unsigned int sh_hist[]; // [kShBins] bins for a, then for b
+    extern __shared__ __align__(8) unsigned char sh_raw[]; // [kLut] doubles, then [kShBins] bins for a and for b
+    double *sh_log = reinterpret_cast<double *>(sh_raw);
+    unsigned int *sh_hist = reinterpret_cast<unsigned int *>(sh_raw + kLut * sizeof(double));
     unsigned int *sh_a = sh_hist, *sh_b = sh_hist + kShBins;
     for (unsigned int k = threadIdx.x; k < (TWO ? 2 : 1) * kShBins; k += kPassThreads) sh_hist[k] = 0u;
-    // dm_a - dm_b = kLn * ln(N_a/N_b) + kRays   (eq. 10), kLn = -2.5/ln 10, kRays = 2.5 log10(n_rays_a/n_rays_b)
-    const double kLn = -2.5 / 2.302585092994046;
-    const double kRays = (n_rays_a == n_rays_b) ? 0.0 : 2.5 * log10(n_rays_a / n_rays_b);
+    if (TWO)
+        for (unsigned int k = threadIdx.x; k < kLut; k += kPassThreads) sh_log[k] = lut[k]; // [0] = -inf, never read
+    const double log_rays = (n_rays_a == n_rays_b) ? 0.0 : log10(n_rays_a / n_rays_b);
     __syncthreads();
 
     Partial p;
@@ -94,12 +87,12 @@ __global__ void __launch_bounds__(kPassThreads, 1) pass_kernel(const unsigned in
     const long long stride = (long long)gridDim.x * kPassThreads * 4;
     unsigned int n_valid = 0, n_empty_a = 0, n_empty_b = 0; // per thread: < 2^31 / (gridDim.x * 1024) pixels each
 
-    auto load4 = [&](long long i, unsigned int (&ca)[4], unsigned int (&cb)[4], int &cnt) {
+    auto load4 = [&](long long i, unsigned int (&ca)[4], unsigned int (&cb)[4]) {
 #pragma unroll
         for (int q = 0; q < 4; ++q) { ca[q] = 0u; cb[q] = 0u; }
-        cnt = i < n ? (int)min(4ll, n - i) : 0;
-        if (cnt == 4 && vec) {
-            const uint4 va = __ldcs(reinterpret_cast<const uint4 *>(a + i)); // streamed: read once
+        if (i >= n) return;
+        if (vec && i + 3 < n) {
+            const uint4 va = __ldcs(reinterpret_cast<const uint4 *>(a + i)); // streamed: every pixel is read once
             ca[0] = va.x; ca[1] = va.y; ca[2] = va.z; ca[3] = va.w;
             if (TWO) {
                 const uint4 vb = __ldcs(reinterpret_cast<const uint4 *>(b + i));
@@ -108,79 +101,73 @@ __global__ void __launch_bounds__(kPassThreads, 1) pass_kernel(const unsigned in
         } else {
 #pragma unroll
             for (int q = 0; q < 4; ++q)
-                if (q < cnt) {
+                if (i + q < n) {
                     ca[q] = a[i + q];
                     if (TWO) cb[q] = b[i + q];
                 }
         }
     };
-    // every thread of the CTA runs the same number of iterations (warp-wide votes inside): cnt = 0 means "no pixels"
-    auto process4 = [&](const unsigned int (&ca)[4], const unsigned int (&cb)[4], int cnt) {
-        unsigned int s_a = 0, s_b = 0;
-        double sv[4];
-        float s2max = 0.f;
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const bool live = q < cnt;
-            if (live) {
-                hist_add(sh_a, hist_a, cap, ca[q]);
-                if (TWO) hist_add(sh_b, hist_b, cap, cb[q]);
-            }
-            s_a += ca[q]; // dead slots hold 0
-            p.max_a = max(p.max_a, ca[q]);
-            n_empty_a += live && (ca[q] == 0);
-            if (TWO) {
-                s_b += cb[q];
-                p.max_b = max(p.max_b, cb[q]);
-                n_empty_b += live && (cb[q] == 0);
-                const bool valid = (ca[q] != 0) & (cb[q] != 0);
-                n_valid += valid;
-                // s = (N_a - N_b)/(N_a + N_b): both exact in fp64; s = 0 for pixels outside the RMS (M1)
-                const double fa = (double)ca[q], fb = (double)cb[q];
-                const double num = fa - fb, den = valid ? fa + fb : 1.0;
-                const double r = recip_int(den);
-                double s = num * r;
-                s = __fma_rn(__fma_rn(-den, s, num), r, s); // one correction step: s within an ulp of num/den
-                sv[q] = valid ? s : 0.0;
-                s2max = fmaxf(s2max, (float)(sv[q] * sv[q]));
-            }
-        }
-        p.sum_a += s_a;
-        if (!TWO) return;
-        p.sum_b += s_b;
-        // how many terms of atanh(s)/s = sum_k s^(2k)/(2k+1) this WARP needs for a relative truncation error < 2^-54
-        // (tail < s2^K/(1 - s2)): s2 <= 2^-12: 5, 2^-8: 7, 2^-6: 9, 2^-4: 14; beyond: two logarithms per pixel
-        const unsigned int key = __reduce_max_sync(0xffffffffu, __float_as_uint(s2max)); // s2 >= 0: bit order = value order
-        const float w = __uint_as_float(key);
-        if (w <= 0.0625f) {
-            const int K = w <= 0x1p-12f ? 5 : (w <= 0x1p-8f ? 7 : (w <= 0x1p-6f ? 9 : 14));
+    auto process4 = [&](long long i, const unsigned int (&ca)[4], const unsigned int (&cb)[4]) {
+        if (i >= n) return;
+        const unsigned int big = ca[0] | ca[1] | ca[2] | ca[3] | cb[0] | cb[1] | cb[2] | cb[3];
+        if (i + 3 < n && big < kLut) {
+            // common case: four pixels, every count inside the log table and the shared-memory bins: no range checks
+            unsigned int s_a = 0, s_b = 0;
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                const double s = sv[q], s2 = s * s;
-                double poly = c_odd_recip[K - 1];
-                for (int k = K - 2; k >= 0; --k) poly = __fma_rn(poly, s2, c_odd_recip[k]);
-                const double d = __fma_rn(kLn * 2.0, s * poly, kRays); // kLn ln(N_a/N_b) + kRays
-                p.ssq += (ca[q] != 0 && cb[q] != 0) ? d * d : 0.0;
-            }
-        } else {
-#pragma unroll
-            for (int q = 0; q < 4; ++q)
-                if (ca[q] != 0 && cb[q] != 0) {
-                    const double d = __fma_rn(kLn, log((double)ca[q]) - log((double)cb[q]), kRays);
-                    p.ssq += d * d;
+                atomicAdd(&sh_a[ca[q]], 1u);
+                if (TWO) atomicAdd(&sh_b[cb[q]], 1u);
+                {
+                    s_a += ca[q];
+                    p.max_a = max(p.max_a, ca[q]);
+                    n_empty_a += (ca[q] == 0);
+                    if (TWO) {
+                        s_b += cb[q];
+                        p.max_b = max(p.max_b, cb[q]);
+                        n_empty_b += (cb[q] == 0);
+                        const bool valid = (ca[q] != 0) & (cb[q] != 0);
+                        // dm_a - dm_b = -2.5 (log10 N_a - log10 N_b - log10(n_rays_a / n_rays_b))   (eq. 10)
+                        const double d = -2.5 * ((sh_log[ca[q]] - sh_log[cb[q]]) - log_rays);
+                        p.ssq += valid ? d * d : 0.0;
+                        n_valid += valid;
+                    }
                 }
+            }
+            p.sum_a += s_a;
+            p.sum_b += s_b;
+            return;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (i + q >= n) break;
+            hist_add(sh_a, hist_a, cap, ca[q]);
+            if (TWO) hist_add(sh_b, hist_b, cap, cb[q]);
+            {
+                p.sum_a += ca[q];
+                p.max_a = max(p.max_a, ca[q]);
+                n_empty_a += (ca[q] == 0);
+                if (TWO) {
+                    p.sum_b += cb[q];
+                    p.max_b = max(p.max_b, cb[q]);
+                    n_empty_b += (cb[q] == 0);
+                    if (ca[q] > 0 && cb[q] > 0) {
+                        const double la = ca[q] < kLut ? sh_log[ca[q]] : log10((double)ca[q]);
+                        const double lb = cb[q] < kLut ? sh_log[cb[q]] : log10((double)cb[q]);
+                        const double d = -2.5 * ((la - lb) - log_rays);
+                        p.ssq += d * d;
+                        n_valid += 1;
+                    }
+                }
+            }
         }
     };
     // two quads in flight per thread: the loads of the second are issued before the first is processed
-    const long long first = ((long long)blockIdx.x * kPassThreads + threadIdx.x) * 4;
-    const long long warp_first = ((long long)blockIdx.x * kPassThreads + (threadIdx.x & ~31)) * 4; // same for the whole warp
-    for (long long off = 0; warp_first + off < n; off += 2 * stride) {
+    for (long long i = ((long long)blockIdx.x * kPassThreads + threadIdx.x) * 4; i < n; i += 2 * stride) {
         unsigned int ca0[4], cb0[4], ca1[4], cb1[4];
-        int c0, c1;
-        load4(first + off, ca0, cb0, c0);
-        load4(first + off + stride, ca1, cb1, c1);
-        process4(ca0, cb0, c0);
-        process4(ca1, cb1, c1);
+        load4(i, ca0, cb0);
+        load4(i + stride, ca1, cb1);
+        process4(i, ca0, cb0);
+        process4(i + stride, ca1, cb1);
     }
     p.n_valid = n_valid; p.n_empty_a = n_empty_a; p.n_empty_b = n_empty_b;
     __syncthreads();
@@ -192,30 +179,32 @@ __global__ void __launch_bounds__(kPassThreads, 1) pass_kernel(const unsigned in
             if (vb) atomicAdd(&hist_b[k], vb);
         }
     }
-    // block reduction in a fixed order: lanes by shuffle tree, then warps in index order
+    {
+        // block reduction in a fixed order: lanes by shuffle tree, then warps in index order
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        p.ssq += __shfl_down_sync(0xffffffffu, p.ssq, o);
-        p.n_valid += __shfl_down_sync(0xffffffffu, p.n_valid, o);
-        p.n_empty_a += __shfl_down_sync(0xffffffffu, p.n_empty_a, o);
-        p.n_empty_b += __shfl_down_sync(0xffffffffu, p.n_empty_b, o);
-        p.sum_a += __shfl_down_sync(0xffffffffu, p.sum_a, o);
-        p.sum_b += __shfl_down_sync(0xffffffffu, p.sum_b, o);
-        p.max_a = max(p.max_a, __shfl_down_sync(0xffffffffu, p.max_a, o));
-        p.max_b = max(p.max_b, __shfl_down_sync(0xffffffffu, p.max_b, o));
-    }
-    __shared__ Partial wp[kPassThreads / 32];
-    if ((threadIdx.x & 31) == 0) wp[threadIdx.x >> 5] = p;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        Partial t = wp[0];
-        for (int w = 1; w < kPassThreads / 32; ++w) {
-            t.ssq += wp[w].ssq;
-            t.n_valid += wp[w].n_valid; t.n_empty_a += wp[w].n_empty_a; t.n_empty_b += wp[w].n_empty_b;
-            t.sum_a += wp[w].sum_a; t.sum_b += wp[w].sum_b;
-            t.max_a = max(t.max_a, wp[w].max_a); t.max_b = max(t.max_b, wp[w].max_b);
+        for (int o = 16; o > 0; o >>= 1) {
+            p.ssq += __shfl_down_sync(0xffffffffu, p.ssq, o);
+            p.n_valid += __shfl_down_sync(0xffffffffu, p.n_valid, o);
+            p.n_empty_a += __shfl_down_sync(0xffffffffu, p.n_empty_a, o);
+            p.n_empty_b += __shfl_down_sync(0xffffffffu, p.n_empty_b, o);
+            p.sum_a += __shfl_down_sync(0xffffffffu, p.sum_a, o);
+            p.sum_b += __shfl_down_sync(0xffffffffu, p.sum_b, o);
+            p.max_a = max(p.max_a, __shfl_down_sync(0xffffffffu, p.max_a, o));
+            p.max_b = max(p.max_b, __shfl_down_sync(0xffffffffu, p.max_b, o));
         }
-        partials[blockIdx.x] = t;
+        __shared__ Partial wp[kPassThreads / 32];
+        if ((threadIdx.x & 31) == 0) wp[threadIdx.x >> 5] = p;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            Partial t = wp[0];
+            for (int w = 1; w < kPassThreads / 32; ++w) {
+                t.ssq += wp[w].ssq;
+                t.n_valid += wp[w].n_valid; t.n_empty_a += wp[w].n_empty_a; t.n_empty_b += wp[w].n_empty_b;
+                t.sum_a += wp[w].sum_a; t.sum_b += wp[w].sum_b;
+                t.max_a = max(t.max_a, wp[w].max_a); t.max_b = max(t.max_b, wp[w].max_b);
+            }
+            partials[blockIdx.x] = t;
+        }
     }
 }
 
@@ -428,7 +417,7 @@ namespace {
 using namespace mlstats;
 
 constexpr int kMaxDevices = 64;
-constexpr size_t kPassSmem = 2 * kShBins * sizeof(unsigned int);
+constexpr size_t kPassSmem = kLut * sizeof(double) + 2 * kShBins * sizeof(unsigned int);
 
 // Everything a call needs on one device, created on first use and kept: no allocation, event creation or
 // synchronisation per call besides the read-back of the result.  Calls are serialised by `lock` (a call ends with a
@@ -445,6 +434,7 @@ struct Scratch {
     unsigned int *tile_sums = nullptr; // [2][n_tiles]
     Partial *partials = nullptr;   // [sm_count]
     Totals *totals = nullptr;
+    double *lut = nullptr;         // [kLut] log10 table, built once
     ml_map_compare_result *d_res = nullptr;
     struct Pinned { ml_map_compare_result res; Totals tot; } *pinned = nullptr;
     unsigned int *map_a = nullptr, *map_b = nullptr; // device copies of host maps
@@ -499,6 +489,7 @@ struct Scratch {
             cudaFuncSetAttribute(pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPassSmem) != cudaSuccess)
             return ML_ERR_CUDA;
         if (cudaMalloc(&partials, (size_t)sm_count * sizeof(Partial)) != cudaSuccess || cudaMalloc(&totals, sizeof(Totals)) != cudaSuccess ||
+            cudaMalloc(&lut, kLut * sizeof(double)) != cudaSuccess ||
             cudaMalloc(&d_res, sizeof(ml_map_compare_result)) != cudaSuccess || cudaMallocHost(&pinned, sizeof(Pinned)) != cudaSuccess) {
             cudaGetLastError();
             return ML_ERR_OOM;
@@ -507,6 +498,8 @@ struct Scratch {
             cudaEventCreate(&evp1) != cudaSuccess)
             return ML_ERR_CUDA;
         if (!set_cap(kCap0)) return ML_ERR_OOM;
+        lut_kernel<<<kLut / 256, 256>>>(lut); // legacy stream; the synchronisation below orders it before every later call
+        if (cudaGetLastError() != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) return ML_ERR_CUDA;
         ready = true;
         return ML_OK;
     }
@@ -555,8 +548,8 @@ int run_pass(Scratch &sc, cudaStream_t s, const uint32_t *a, const uint32_t *b, 
     if (cudaEventRecord(sc.ev0, s) != cudaSuccess || cudaMemsetAsync(sc.zeroed, 0, sc.zeroed_bytes(two), s) != cudaSuccess ||
         cudaEventRecord(sc.evp0, s) != cudaSuccess)
         return ML_ERR_CUDA;
-    if (two) pass_kernel<true><<<grid, kPassThreads, kPassSmem, s>>>(*da, *db, n, na, nb, sc.hist, sc.hist + sc.cap, sc.cap, sc.partials);
-    else pass_kernel<false><<<grid, kPassThreads, kPassSmem, s>>>(*da, nullptr, n, na, nb, sc.hist, nullptr, sc.cap, sc.partials);
+    if (two) pass_kernel<true><<<grid, kPassThreads, kPassSmem, s>>>(*da, *db, n, na, nb, sc.hist, sc.hist + sc.cap, sc.cap, sc.partials, sc.lut);
+    else pass_kernel<false><<<grid, kPassThreads, kPassSmem, s>>>(*da, nullptr, n, na, nb, sc.hist, nullptr, sc.cap, sc.partials, sc.lut);
     if (cudaGetLastError() != cudaSuccess || cudaEventRecord(sc.evp1, s) != cudaSuccess) return ML_ERR_CUDA;
     reduce_partials_kernel<<<1, 32, 0, s>>>(sc.partials, grid, sc.cap, sc.totals);
     return cudaGetLastError() == cudaSuccess ? ML_OK : ML_ERR_CUDA;

@@ -102,7 +102,8 @@ typedef struct {
 typedef struct {
     uint64_t rays_shot;    /* rays processed by the last shoot (sum over accumulated regions) */
     uint64_t rays_in_map;  /* rays counted into the map                                       */
-    uint64_t rays_dropped; /* rays whose y was not finite (ray on a lens): not binned         */
+    uint64_t rays_dropped; /* rays whose y was not finite: not binned.  A ray exactly ON a lens is dropped in
+                              ML_PREC_FP64; in the FP32 modes it does not see that one lens (R12)     */
     uint64_t interactions; /* rays_shot * n_lenses (eq.6 without N_FLOP)       */
     uint64_t kernel_launches; /* launches of the shoot kernel since the map was last zeroed   */
     double kernel_ms;      /* device time of those launches, CUDA events on the ctx stream    */

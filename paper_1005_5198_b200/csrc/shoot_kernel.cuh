@@ -24,9 +24,8 @@
 //
 // Summation order and precision:
 //   lenses in index order; FP32 partial sums over groups of KF consecutive lenses (groups
-//   aligned to multiples of KF in lens index; a trailing group of fewer than KF/2 lenses is
-//   joined to the group before it when that group lies in the same 512-lens chunk) are added,
-//   in order, to one fp64 accumulator per ray and component.  With Real = double the partials are fp64 too
+//   aligned to multiples of KF in lens index) are added, in order, to one fp64
+//   accumulator per ray and component.  With Real = double the partials are fp64 too
 //   and the reciprocal is an IEEE division.
 //   Every FP32 operation is written with an explicit-rounding intrinsic so that the
 //   compiler can neither contract nor reassociate: the arithmetic of a ray does not
@@ -167,22 +166,8 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
         }
         return w;
     };
-    // per-column / per-row quantities once per thread: ray index as an exact double and "inside the requested region" bits
-    const double ib = (double)(ti * TW), jb = (double)(tj * TH);
-    double fi[RX], fj[RY];
-    unsigned int colmask = 0u, rowmask = 0u;
-#pragma unroll
-    for (int c = 0; c < RX; ++c) {
-        const long long i = ti * TW + lane * RX + c;
-        fi[c] = ib + (double)(lane * RX + c); // = (double)i exactly
-        colmask |= ((i >= p.i0) && (i < p.i1)) ? (1u << c) : 0u;
-    }
-#pragma unroll
-    for (int r = 0; r < RY; ++r) {
-        const long long j = tj * TH + warp * RY + r;
-        fj[r] = jb + (double)(warp * RY + r);
-        rowmask |= ((j >= p.j0) && (j < p.j1)) ? (1u << r) : 0u;
-    }
+    // ray indices as exact doubles: (double)(ti*TW) + small integer = (double)i, no 64-bit conversions per ray
+    const double ib = (double)(ti * TW) + (double)(lane * RX), jb = (double)(tj * TH) + (double)(warp * RY);
     if (CAPTURE) {
 #pragma unroll
         for (int r = 0; r < RY; ++r)
@@ -191,11 +176,11 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
                 double x1, x2;
                 if (RANDOM) { // the ray's own position in its cell (the draw of the prologue)
                     const double2 w = draw(r, c);
-                    x1 = (fi[c] + w.x - (p.half1 + 0.5)) * p.delta;
-                    x2 = (fj[r] + w.y - (p.half2 + 0.5)) * p.delta;
+                    x1 = ((ib + (double)c) + w.x - (p.half1 + 0.5)) * p.delta;
+                    x2 = ((jb + (double)r) + w.y - (p.half2 + 0.5)) * p.delta;
                 } else {
-                    x1 = (fi[c] - p.half1) * p.delta;
-                    x2 = (fj[r] - p.half2) * p.delta;
+                    x1 = ((ib + (double)c) - p.half1) * p.delta;
+                    x2 = ((jb + (double)r) - p.half2) * p.delta;
                 }
                 const double y1 = p.c1 * x1 - Sx[r][c];
                 const double y2 = p.c2 * x2 - Sy[r][c];
@@ -209,27 +194,36 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
         return;
     }
     // ---- a4 + a5: macro terms folded into the pixel coordinate, binning
-    double U1[RX], U2[RY];
-    if (!RANDOM) {
+    // "inside the requested region" bits per column / row, and the x-part of the pixel coordinate per column
+    unsigned int colmask = 0u, rowmask = 0u;
+    double U1[RX];
 #pragma unroll
-        for (int c = 0; c < RX; ++c) U1[c] = __fma_rn((fi[c] - p.half1) * p.delta, p.k1, p.hoff);
+    for (int c = 0; c < RX; ++c) {
+        const long long i = ti * TW + lane * RX + c;
+        colmask |= ((i >= p.i0) && (i < p.i1)) ? (1u << c) : 0u;
+        if (!RANDOM) U1[c] = __fma_rn(((ib + (double)c) - p.half1) * p.delta, p.k1, p.hoff);
+    }
 #pragma unroll
-        for (int r = 0; r < RY; ++r) U2[r] = __fma_rn((fj[r] - p.half2) * p.delta, p.k2, p.hoff);
+    for (int r = 0; r < RY; ++r) {
+        const long long j = tj * TH + warp * RY + r;
+        rowmask |= ((j >= p.j0) && (j < p.j1)) ? (1u << r) : 0u;
     }
     const unsigned int n_pix_u = (unsigned int)p.n_pix;
     const double nip = -p.inv_pixel;
 #pragma unroll
     for (int r = 0; r < RY; ++r) {
+        double U2 = 0.0;
+        if (!RANDOM) U2 = __fma_rn(((jb + (double)r) - p.half2) * p.delta, p.k2, p.hoff);
 #pragma unroll
         for (int c = 0; c < RX; ++c) {
             double b1, b2;
             if (RANDOM) {
                 const double2 w = draw(r, c);
-                b1 = __fma_rn((fi[c] + w.x - (p.half1 + 0.5)) * p.delta, p.k1, p.hoff);
-                b2 = __fma_rn((fj[r] + w.y - (p.half2 + 0.5)) * p.delta, p.k2, p.hoff);
+                b1 = __fma_rn(((ib + (double)c) + w.x - (p.half1 + 0.5)) * p.delta, p.k1, p.hoff);
+                b2 = __fma_rn(((jb + (double)r) + w.y - (p.half2 + 0.5)) * p.delta, p.k2, p.hoff);
             } else {
                 b1 = U1[c];
-                b2 = U2[r];
+                b2 = U2;
             }
             const double u1 = __fma_rn(Sx[r][c], nip, b1);
             const double u2 = __fma_rn(Sy[r][c], nip, b2);
@@ -444,9 +438,8 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
         const int cntp = (cnt + 7) & ~7; // padded with zero-contribution lenses
         const Real2 *ls = lens_s[buf];
         const Real *ms = mass_s[buf];
-        for (int k0 = 0, kend; k0 < cntp; k0 = kend) {
-            kend = min(k0 + KF, cntp);
-            if (cntp - kend < KF / 2) kend = cntp; // a trailing group shorter than KF/2 joins the group before it
+        for (int k0 = 0; k0 < cntp; k0 += KF) {
+            const int kend = min(k0 + KF, cntp);
 #pragma unroll 1
             for (int k = k0; k < kend; k += 2) {
 #pragma unroll
@@ -535,7 +528,13 @@ template <int RY> struct PipeRegs {
     float2 R[RY];
 };
 
-template <int SHARED, int KF, int WARPS, int MINB, bool SCALAR_DY, bool CAPTURE, bool MASS = false, bool NEWTON = false>
+// TUNE: source-order knobs that change nothing in the arithmetic of a ray (same operations, same operands, same
+// rounding) but steer ptxas towards different instruction schedules of the loop; the value the library uses was
+// picked by measurement on the B200.  bit 0: pipeline two lenses ahead instead of
+// one; bits 1-2: order of the four accumulations of a row; bit 3: 1/r^2 of pair B after the accumulations of pair A;
+// bit 4: rows in reverse order in stage 2; bit 5: rows in reverse order in stage 1; bit 6: stage 1 forms r^2 of
+// all rows before the first reciprocal; bit 7: stage 2 forms every 1/r^2 before the first accumulation.
+template <int SHARED, int KF, int WARPS, int MINB, bool SCALAR_DY, bool CAPTURE, bool MASS = false, bool NEWTON = false, int TUNE = 0>
 __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const ShootParams p)
 {
     constexpr int RX = 4, RY = 4;
@@ -620,8 +619,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
         s.dxA = __fadd2_rn(oxA, nlx);
         s.dxB = __fadd2_rn(oxB, nlx);
         const float2 qA = __ffma2_rn(s.dxA, s.dxA, eps2), qB = __ffma2_rn(s.dxB, s.dxB, eps2);
-#pragma unroll
-        for (int r = 0; r < RY; ++r) {
+        auto row_r2 = [&](int r) {
             float2 dy;
             if (SCALAR_DY) {
                 s.dy[r] = __fadd_rn(oy[r], l.z);
@@ -632,6 +630,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
             }
             s.r2A[r] = __ffma2_rn(dy, dy, qA);
             s.r2B[r] = __ffma2_rn(dy, dy, qB);
+        };
+        auto row_rcp = [&](int r) {
             if (r < SHARED) {
                 const float2 P = __fmul2_rn(s.r2A[r], s.r2B[r]);
                 s.R[r].x = rcp_approx(P.x);
@@ -640,14 +640,26 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
                 s.r2A[r].x = rcp_approx(s.r2A[r].x); s.r2A[r].y = rcp_approx(s.r2A[r].y);
                 s.r2B[r].x = rcp_approx(s.r2B[r].x); s.r2B[r].y = rcp_approx(s.r2B[r].y);
             }
+        };
+        if (TUNE & 64) { // all r^2 first, then the products and reciprocals
+#pragma unroll
+            for (int rr = 0; rr < RY; ++rr) row_r2((TUNE & 32) ? RY - 1 - rr : rr);
+#pragma unroll
+            for (int rr = 0; rr < RY; ++rr) row_rcp((TUNE & 32) ? RY - 1 - rr : rr);
+        } else {
+#pragma unroll
+            for (int rr = 0; rr < RY; ++rr) {
+                const int r = (TUNE & 32) ? RY - 1 - rr : rr;
+                row_r2(r);
+                row_rcp(r);
+            }
         }
     };
     auto stage2 = [&](const PipeRegs<RY> &s) {
-#pragma unroll
-        for (int r = 0; r < RY; ++r) {
-            float2 iA, iB;
+        float2 iAs[RY], iBs[RY];
+        auto inv_r2 = [&](int r, float2 &iA, float2 &iB, float2 &R, bool both) {
+            R = s.R[r];
             if (r < SHARED) {
-                float2 R = s.R[r];
                 if (NEWTON) { // one Newton-Raphson step on the shared reciprocal: R <- R + R (1 - P R), P = r2A r2B
                     const float2 P = __fmul2_rn(s.r2A[r], s.r2B[r]);
                     const float2 e = __ffma2_rn(make_float2(-P.x, -P.y), R, make_float2(1.f, 1.f));
@@ -655,16 +667,56 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
                 }
                 if (MASS) R = __fmul2_rn(R, make_float2(s.m, s.m)); // m_i / (r2A r2B)
                 iA = __fmul2_rn(R, s.r2B[r]);
-                iB = __fmul2_rn(R, s.r2A[r]);
+                if (both) iB = __fmul2_rn(R, s.r2A[r]);
             } else {
                 iA = MASS ? __fmul2_rn(s.r2A[r], make_float2(s.m, s.m)) : s.r2A[r];
                 iB = MASS ? __fmul2_rn(s.r2B[r], make_float2(s.m, s.m)) : s.r2B[r];
             }
+        };
+        if (TUNE & 128) {
+#pragma unroll
+            for (int rr = 0; rr < RY; ++rr) {
+                const int r = (TUNE & 16) ? RY - 1 - rr : rr;
+                float2 R;
+                inv_r2(r, iAs[r], iBs[r], R, true);
+            }
+        }
+#pragma unroll
+        for (int rr = 0; rr < RY; ++rr) {
+            const int r = (TUNE & 16) ? RY - 1 - rr : rr;
+            float2 iA, iB, R;
+            const bool late_b = (TUNE & 8) && !(TUNE & 128) && r < SHARED;
+            if (TUNE & 128) { iA = iAs[r]; iB = iBs[r]; }
+            else inv_r2(r, iA, iB, R, !late_b);
             const float2 dy = make_float2(s.dy[r], s.dy[r]);
-            sxA[r] = __ffma2_rn(s.dxA, iA, sxA[r]);
-            sxB[r] = __ffma2_rn(s.dxB, iB, sxB[r]);
-            syA[r] = __ffma2_rn(dy, iA, syA[r]);
-            syB[r] = __ffma2_rn(dy, iB, syB[r]);
+            constexpr int ORD = (TUNE >> 1) & 3;
+            if (late_b) { // pair A first, then 1/r^2 of pair B and its accumulations
+                if (ORD & 1) { syA[r] = __ffma2_rn(dy, iA, syA[r]); sxA[r] = __ffma2_rn(s.dxA, iA, sxA[r]); }
+                else { sxA[r] = __ffma2_rn(s.dxA, iA, sxA[r]); syA[r] = __ffma2_rn(dy, iA, syA[r]); }
+                iB = __fmul2_rn(R, s.r2A[r]);
+                if (ORD & 2) { syB[r] = __ffma2_rn(dy, iB, syB[r]); sxB[r] = __ffma2_rn(s.dxB, iB, sxB[r]); }
+                else { sxB[r] = __ffma2_rn(s.dxB, iB, sxB[r]); syB[r] = __ffma2_rn(dy, iB, syB[r]); }
+            } else if (ORD == 0) {
+                sxA[r] = __ffma2_rn(s.dxA, iA, sxA[r]);
+                sxB[r] = __ffma2_rn(s.dxB, iB, sxB[r]);
+                syA[r] = __ffma2_rn(dy, iA, syA[r]);
+                syB[r] = __ffma2_rn(dy, iB, syB[r]);
+            } else if (ORD == 1) {
+                sxA[r] = __ffma2_rn(s.dxA, iA, sxA[r]);
+                syA[r] = __ffma2_rn(dy, iA, syA[r]);
+                sxB[r] = __ffma2_rn(s.dxB, iB, sxB[r]);
+                syB[r] = __ffma2_rn(dy, iB, syB[r]);
+            } else if (ORD == 2) {
+                syA[r] = __ffma2_rn(dy, iA, syA[r]);
+                syB[r] = __ffma2_rn(dy, iB, syB[r]);
+                sxA[r] = __ffma2_rn(s.dxA, iA, sxA[r]);
+                sxB[r] = __ffma2_rn(s.dxB, iB, sxB[r]);
+            } else {
+                syA[r] = __ffma2_rn(dy, iA, syA[r]);
+                sxA[r] = __ffma2_rn(s.dxA, iA, sxA[r]);
+                syB[r] = __ffma2_rn(dy, iB, syB[r]);
+                sxB[r] = __ffma2_rn(s.dxB, iB, sxB[r]);
+            }
         }
     };
 
@@ -679,15 +731,22 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
         auto mass_of = [&](int k) { return MASS ? ms[k] : 1.f; };
         PipeRegs<RY> a, b;
         stage1(ls[0], mass_of(0), a);
-        for (int k0 = 0, kend; k0 < cntp; k0 = kend) {
-            kend = min(k0 + KF, cntp);
-            if (cntp - kend < KF / 2) kend = cntp; // a trailing group shorter than KF/2 joins the group before it
+        if (TUNE & 1) stage1(ls[1], mass_of(1), b);
+        for (int k0 = 0; k0 < cntp; k0 += KF) {
+            const int kend = min(k0 + KF, cntp);
 #pragma unroll 1
             for (int k = k0; k < kend; k += 2) {
-                stage1(ls[k + 1], mass_of(k + 1), b);
-                stage2(a);
-                stage1(ls[k + 2], mass_of(k + 2), a);
-                stage2(b);
+                if (TUNE & 1) { // lenses k, k+1 are staged; stage k+2, k+3 (<= cntp + 1: a padding lens) behind their use
+                    stage2(a);
+                    stage1(ls[k + 2], mass_of(k + 2), a);
+                    stage2(b);
+                    stage1(ls[k + 3], mass_of(k + 3), b);
+                } else {
+                    stage1(ls[k + 1], mass_of(k + 1), b);
+                    stage2(a);
+                    stage1(ls[k + 2], mass_of(k + 2), a);
+                    stage2(b);
+                }
             }
 #pragma unroll
             for (int r = 0; r < RY; ++r) {
@@ -887,9 +946,8 @@ __global__ void __launch_bounds__(kRandWarps * 32, MINB) shoot_kernel_rpipe(cons
         const std::integral_constant<bool, false> even;
         const std::integral_constant<bool, true> odd;
         stage1(even, ls[0], mass_of(0), a);
-        for (int k0 = 0, kend; k0 < cntp; k0 = kend) {
-            kend = min(k0 + KF, cntp);
-            if (cntp - kend < KF / 2) kend = cntp; // a trailing group shorter than KF/2 joins the group before it
+        for (int k0 = 0; k0 < cntp; k0 += KF) {
+            const int kend = min(k0 + KF, cntp);
 #pragma unroll 1
             for (int k = k0; k < kend; k += 2) {
                 stage1(odd, ls[k + 1], mass_of(k + 1), b);

@@ -155,9 +155,11 @@ def test_state_and_argument_errors_on_a_live_context():
 
 @pytest.mark.parametrize("precision", ALL)
 def test_ray_on_a_lens_does_not_poison_the_map(precision):
-    """Reading R12: a ray coincident with a lens is dropped (oracle) or flung far outside
-    the map (tile-local FP32 coordinates differ in the last bit); either way it is not
-    binned, nothing is NaN-poisoned and every ray is accounted for."""
+    """Reading R12: the deflection of a ray that sits exactly on a point mass is undefined.  The oracle and the fp64
+    kernel find r^2 = 0, get a non-finite position and DROP the ray (counted in rays_dropped, not binned).  The FP32
+    kernels hold ray and lens in tile-local FP32 coordinates, where the two coincide as well: r^2 = 0 + 2^-80, the term
+    d/r^2 = 0 * 2^80 = 0, i.e. the ray does not see that one lens and is binned from the other N* - 1 (its partner in
+    the shared reciprocal is untouched).  Either way nothing is NaN-poisoned and every ray is accounted for."""
     p = SMALL
     g = oracle.geometry(*problem_args(p))
     xy = lens_disk(40, g.r_star, 5)
@@ -172,6 +174,12 @@ def test_ray_on_a_lens_does_not_poison_the_map(precision):
         assert st["rays_shot"] == g.n1 * g.n2
         assert st["rays_in_map"] + st["rays_dropped"] <= st["rays_shot"]
         check_maps(p, m.counts(), st, omap, ost)
+        y = m.probe([i], [j])[0]
+        y_rest = oracle.deflect_points(p.gamma, g.kappa_c, xy[1:], np.array([xy[0]]))[0]   # the same ray without lens 0
+        if precision == ml.ML_PREC_FP64:
+            assert st["rays_dropped"] == 1 and np.isnan(y).all()
+        else:
+            assert st["rays_dropped"] == 0 and np.abs(y - y_rest).max() < 1e-3 * g.pixel
 
 
 def test_caller_owned_torch_map_and_stream():

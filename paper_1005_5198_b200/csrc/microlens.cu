@@ -67,9 +67,12 @@ constexpr int WARPS_T = 4, SHARED_T = 4, MINB_T = 3; // FP32_TILED: 128-thread C
 // source-order knobs of shoot_kernel_pipe (same arithmetic, different ptxas schedule), picked by a sweep of all 256
 // values on the B200: 44 = rows reversed in stage 1, pair B's 1/r^2 after pair A's accumulations, sy before sx
 // (C2 slab 72.4 -> 73.7 % of FP32 peak, C4 slab 73.3 -> 74.9 %, N* = 135: 66.2 -> 67.2 %)
+// The instantiations with masses and with the Newton step have other optima (same sweep: masses 4 -> 65.4 / 66.3 %,
+// against 63.6 / 64.3 % with 44; Newton 2 -> 56.3 / 56.6 %).
 #ifndef ML_PIPE_TUNE
 #define ML_PIPE_TUNE 44
 #endif
+constexpr int tune_of(bool mass, bool newton) { return newton ? 2 : (mass ? 4 : ML_PIPE_TUNE); }
 constexpr int KFCP = 16;                   // FP32_COMPENSATED, regular grid: the pipe kernel with a Newton step
 constexpr int RXD = 4, RYD = 2, KFD = 64;  // FP64
 
@@ -92,17 +95,22 @@ template <bool CAPTURE, bool MASS> cudaError_t launch_m(int precision, dim3 g, c
         shoot_kernel<double, RXD, RYD, KFD, false, CAPTURE, MASS><<<g, kThreads, 0, s>>>(p);
         break;
     case ML_PREC_FP32_COMPENSATED:
-        shoot_kernel_pipe<SHARED_T, KFCP, WARPS_T, MINB_T, true, CAPTURE, MASS, true, ML_PIPE_TUNE><<<g, WARPS_T * 32, 0, s>>>(p);
+        shoot_kernel_pipe<SHARED_T, KFCP, WARPS_T, MINB_T, true, CAPTURE, MASS, true, tune_of(MASS, true)><<<g, WARPS_T * 32, 0, s>>>(p);
         break;
     default:
-        shoot_kernel_pipe<SHARED_T, KFF, WARPS_T, MINB_T, true, CAPTURE, MASS, false, ML_PIPE_TUNE><<<g, WARPS_T * 32, 0, s>>>(p);
+        shoot_kernel_pipe<SHARED_T, KFF, WARPS_T, MINB_T, true, CAPTURE, MASS, false, tune_of(MASS, false)><<<g, WARPS_T * 32, 0, s>>>(p);
         break;
     }
     return cudaGetLastError();
 }
 
+// shoot_kernel_rpipe: own reciprocals on the last row of every lens (OWN = 2) and source-order knobs 10, from a sweep of
+// OWN x TUNE on the B200 (C2 slab: 53.7 % of FP32 peak with everything shared, 56.8 % with these; C4 slab 55.5 -> 59.0 %)
 #ifndef ML_RPIPE_OWN
-#define ML_RPIPE_OWN 1 // see shoot_kernel_rpipe: own reciprocals on the last row of odd lenses
+#define ML_RPIPE_OWN 2
+#endif
+#ifndef ML_RPIPE_TUNE
+#define ML_RPIPE_TUNE 10
 #endif
 // random ray positions (reading R17): the packed random-ray kernel in the FP32 modes, the generic
 // kernel with per-ray offsets in fp64
@@ -111,12 +119,12 @@ template <int KF, bool CAPTURE, bool MASS, bool NEWTON> cudaError_t launch_rpipe
     constexpr size_t smem = rpipe_smem_bytes(MASS);
     static bool opted_in = false; // more than 48 KB of dynamic shared memory needs the opt-in once per function
     if (!opted_in) {
-        const cudaError_t e = cudaFuncSetAttribute(shoot_kernel_rpipe<KF, 2, CAPTURE, MASS, NEWTON, ML_RPIPE_OWN>,
+        const cudaError_t e = cudaFuncSetAttribute(shoot_kernel_rpipe<KF, 2, CAPTURE, MASS, NEWTON, ML_RPIPE_OWN, ML_RPIPE_TUNE>,
                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         opted_in = true;
     }
-    shoot_kernel_rpipe<KF, 2, CAPTURE, MASS, NEWTON, ML_RPIPE_OWN><<<g, kRandWarps * 32, smem, s>>>(p);
+    shoot_kernel_rpipe<KF, 2, CAPTURE, MASS, NEWTON, ML_RPIPE_OWN, ML_RPIPE_TUNE><<<g, kRandWarps * 32, smem, s>>>(p);
     return cudaGetLastError();
 }
 

@@ -534,6 +534,8 @@ template <int RY> struct PipeRegs {
 // one; bits 1-2: order of the four accumulations of a row; bit 3: 1/r^2 of pair B after the accumulations of pair A;
 // bit 4: rows in reverse order in stage 2; bit 5: rows in reverse order in stage 1; bit 6: stage 1 forms r^2 of
 // all rows before the first reciprocal; bit 7: stage 2 forms every 1/r^2 before the first accumulation.
+// bit 8 does change the arithmetic (shoot and capture instantiations alike): on the last row of every odd lens the two
+// ray pairs take their own reciprocals (4 MUFU.RCP) instead of the shared one (2 MUFU.RCP + 3 FMUL2).
 template <int SHARED, int KF, int WARPS, int MINB, bool SCALAR_DY, bool CAPTURE, bool MASS = false, bool NEWTON = false, int TUNE = 0>
 __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const ShootParams p)
 {
@@ -613,7 +615,10 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
     __syncthreads();
 
     const float2 eps2 = make_float2(0x1p-80f, 0x1p-80f);
-    auto stage1 = [&](const float4 l, const float m, PipeRegs<RY> &s) {
+    static_assert(!(NEWTON && ((TUNE & 256) || SHARED < RY)), "the Newton step is written for shared reciprocals only");
+    // rows whose two ray pairs share one reciprocal: all SHARED first rows, except (TUNE bit 8) the last row of odd lenses
+    auto shares = [](int r, bool odd) { return r < SHARED && !((TUNE & 256) && odd && r == RY - 1); };
+    auto stage1 = [&](auto odd, const float4 l, const float m, PipeRegs<RY> &s) {
         const float2 nlx = make_float2(l.x, l.y), nly = make_float2(l.z, l.w);
         s.m = m;
         s.dxA = __fadd2_rn(oxA, nlx);
@@ -632,7 +637,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
             s.r2B[r] = __ffma2_rn(dy, dy, qB);
         };
         auto row_rcp = [&](int r) {
-            if (r < SHARED) {
+            if (shares(r, decltype(odd)::value)) {
                 const float2 P = __fmul2_rn(s.r2A[r], s.r2B[r]);
                 s.R[r].x = rcp_approx(P.x);
                 s.R[r].y = rcp_approx(P.y);
@@ -655,11 +660,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
             }
         }
     };
-    auto stage2 = [&](const PipeRegs<RY> &s) {
+    auto stage2 = [&](auto odd, const PipeRegs<RY> &s) {
         float2 iAs[RY], iBs[RY];
         auto inv_r2 = [&](int r, float2 &iA, float2 &iB, float2 &R, bool both) {
             R = s.R[r];
-            if (r < SHARED) {
+            if (shares(r, decltype(odd)::value)) {
                 if (NEWTON) { // one Newton-Raphson step on the shared reciprocal: R <- R + R (1 - P R), P = r2A r2B
                     const float2 P = __fmul2_rn(s.r2A[r], s.r2B[r]);
                     const float2 e = __ffma2_rn(make_float2(-P.x, -P.y), R, make_float2(1.f, 1.f));
@@ -685,7 +690,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
         for (int rr = 0; rr < RY; ++rr) {
             const int r = (TUNE & 16) ? RY - 1 - rr : rr;
             float2 iA, iB, R;
-            const bool late_b = (TUNE & 8) && !(TUNE & 128) && r < SHARED;
+            const bool late_b = (TUNE & 8) && !(TUNE & 128) && shares(r, decltype(odd)::value);
             if (TUNE & 128) { iA = iAs[r]; iB = iBs[r]; }
             else inv_r2(r, iA, iB, R, !late_b);
             const float2 dy = make_float2(s.dy[r], s.dy[r]);
@@ -729,23 +734,25 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) shoot_kernel_pipe(const Shoo
         const float4 *ls = lens_s[buf];
         const float *ms = mass_s[buf];
         auto mass_of = [&](int k) { return MASS ? ms[k] : 1.f; };
-        PipeRegs<RY> a, b;
-        stage1(ls[0], mass_of(0), a);
-        if (TUNE & 1) stage1(ls[1], mass_of(1), b);
+        PipeRegs<RY> a, b; // a: even lenses of the chunk, b: odd lenses
+        const std::integral_constant<bool, false> even;
+        const std::integral_constant<bool, true> odd;
+        stage1(even, ls[0], mass_of(0), a);
+        if (TUNE & 1) stage1(odd, ls[1], mass_of(1), b);
         for (int k0 = 0; k0 < cntp; k0 += KF) {
             const int kend = min(k0 + KF, cntp);
 #pragma unroll 1
             for (int k = k0; k < kend; k += 2) {
                 if (TUNE & 1) { // lenses k, k+1 are staged; stage k+2, k+3 (<= cntp + 1: a padding lens) behind their use
-                    stage2(a);
-                    stage1(ls[k + 2], mass_of(k + 2), a);
-                    stage2(b);
-                    stage1(ls[k + 3], mass_of(k + 3), b);
+                    stage2(even, a);
+                    stage1(even, ls[k + 2], mass_of(k + 2), a);
+                    stage2(odd, b);
+                    stage1(odd, ls[k + 3], mass_of(k + 3), b);
                 } else {
-                    stage1(ls[k + 1], mass_of(k + 1), b);
-                    stage2(a);
-                    stage1(ls[k + 2], mass_of(k + 2), a);
-                    stage2(b);
+                    stage1(odd, ls[k + 1], mass_of(k + 1), b);
+                    stage2(even, a);
+                    stage1(even, ls[k + 2], mass_of(k + 2), a);
+                    stage2(odd, b);
                 }
             }
 #pragma unroll
@@ -793,9 +800,11 @@ constexpr size_t rpipe_smem_bytes(bool mass)
 }
 
 // OWN = 1: on the last row of every odd lens the two ray pairs take their own reciprocals (4 MUFU, no FMUL2) instead
-// of the shared one (2 MUFU + 3 FMUL2): the XU pipe has room for a quarter more reciprocals (61 % busy instead of 48 %)
-// and the FMA pipe, which bounds the loop, loses 3 of its 60 packed instructions per lens pair.
-template <int KF, int MINB, bool CAPTURE, bool MASS = false, bool NEWTON = false, int OWN = 1>
+// of the shared one (2 MUFU + 3 FMUL2): the XU pipe has room for more reciprocals (48 % busy with everything shared) and
+// the FMA pipe, which bounds the loop, loses 3 of its 60 packed instructions per lens pair.
+// OWN = 2: the same on the last row of every lens.  TUNE: source-order knobs as in shoot_kernel_pipe (bits 0-1: order
+// of the four accumulations of a row; bit 2 / bit 3: rows in reverse order in stage 2 / stage 1).
+template <int KF, int MINB, bool CAPTURE, bool MASS = false, bool NEWTON = false, int OWN = 1, int TUNE = 0>
 __global__ void __launch_bounds__(kRandWarps * 32, MINB) shoot_kernel_rpipe(const ShootParams p)
 {
     constexpr int RX = 4, RY = kRandRY, WARPS = kRandWarps;
@@ -889,14 +898,15 @@ __global__ void __launch_bounds__(kRandWarps * 32, MINB) shoot_kernel_rpipe(cons
         const float2 nlx = make_float2(l.x, l.y), nly = make_float2(l.z, l.w);
         s.m = m;
 #pragma unroll
-        for (int r = 0; r < RY; ++r) {
+        for (int rr = 0; rr < RY; ++rr) {
+            const int r = (TUNE & 8) ? RY - 1 - rr : rr;
             s.dxA[r] = __fadd2_rn(oxA[r], nlx);
             s.dxB[r] = __fadd2_rn(oxB[r], nlx);
             s.dyA[r] = __fadd2_rn(oyA[r], nly);
             s.dyB[r] = __fadd2_rn(oyB[r], nly);
             s.r2A[r] = __ffma2_rn(s.dyA[r], s.dyA[r], __ffma2_rn(s.dxA[r], s.dxA[r], eps2));
             s.r2B[r] = __ffma2_rn(s.dyB[r], s.dyB[r], __ffma2_rn(s.dxB[r], s.dxB[r], eps2));
-            if (OWN && decltype(odd)::value && r == RY - 1) {
+            if (r == RY - 1 && (OWN == 2 || (OWN == 1 && decltype(odd)::value))) {
                 s.R[r].x = rcp_approx(s.r2A[r].x); s.R[r].y = rcp_approx(s.r2A[r].y);
                 s.Rb[r].x = rcp_approx(s.r2B[r].x); s.Rb[r].y = rcp_approx(s.r2B[r].y);
             } else {
@@ -912,9 +922,10 @@ __global__ void __launch_bounds__(kRandWarps * 32, MINB) shoot_kernel_rpipe(cons
     };
     auto stage2 = [&](auto odd, const RPipeRegs<RY> &s) {
 #pragma unroll
-        for (int r = 0; r < RY; ++r) {
+        for (int rr = 0; rr < RY; ++rr) {
+            const int r = (TUNE & 4) ? RY - 1 - rr : rr;
             float2 iA, iB;
-            if (OWN && decltype(odd)::value && r == RY - 1) {
+            if (r == RY - 1 && (OWN == 2 || (OWN == 1 && decltype(odd)::value))) {
                 iA = s.R[r];
                 iB = s.Rb[r];
                 if (NEWTON) { iA = newton(s.r2A[r], iA); iB = newton(s.r2B[r], iB); }
@@ -926,10 +937,28 @@ __global__ void __launch_bounds__(kRandWarps * 32, MINB) shoot_kernel_rpipe(cons
                 iA = __fmul2_rn(R, s.r2B[r]);
                 iB = __fmul2_rn(R, s.r2A[r]);
             }
-            sxA[r] = __ffma2_rn(s.dxA[r], iA, sxA[r]);
-            syA[r] = __ffma2_rn(s.dyA[r], iA, syA[r]);
-            sxB[r] = __ffma2_rn(s.dxB[r], iB, sxB[r]);
-            syB[r] = __ffma2_rn(s.dyB[r], iB, syB[r]);
+            constexpr int ORD = TUNE & 3;
+            if (ORD == 0) {
+                sxA[r] = __ffma2_rn(s.dxA[r], iA, sxA[r]);
+                syA[r] = __ffma2_rn(s.dyA[r], iA, syA[r]);
+                sxB[r] = __ffma2_rn(s.dxB[r], iB, sxB[r]);
+                syB[r] = __ffma2_rn(s.dyB[r], iB, syB[r]);
+            } else if (ORD == 1) {
+                sxA[r] = __ffma2_rn(s.dxA[r], iA, sxA[r]);
+                sxB[r] = __ffma2_rn(s.dxB[r], iB, sxB[r]);
+                syA[r] = __ffma2_rn(s.dyA[r], iA, syA[r]);
+                syB[r] = __ffma2_rn(s.dyB[r], iB, syB[r]);
+            } else if (ORD == 2) {
+                syA[r] = __ffma2_rn(s.dyA[r], iA, syA[r]);
+                syB[r] = __ffma2_rn(s.dyB[r], iB, syB[r]);
+                sxA[r] = __ffma2_rn(s.dxA[r], iA, sxA[r]);
+                sxB[r] = __ffma2_rn(s.dxB[r], iB, sxB[r]);
+            } else {
+                syA[r] = __ffma2_rn(s.dyA[r], iA, syA[r]);
+                sxA[r] = __ffma2_rn(s.dxA[r], iA, sxA[r]);
+                syB[r] = __ffma2_rn(s.dyB[r], iB, syB[r]);
+                sxB[r] = __ffma2_rn(s.dxB[r], iB, sxB[r]);
+            }
         }
     };
 

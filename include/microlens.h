@@ -171,7 +171,9 @@ int ml_get_map(const ml_ctx *ctx, uint32_t *out, size_t out_len);
 int ml_get_map_device(const ml_ctx *ctx, void **dptr);
 
 /* Use caller-owned DEVICE memory (>= n_pix^2 uint32, e.g. a torch tensor) as the map
- * from now on; NULL returns to the library's own buffer.  The caller keeps ownership. */
+ * from now on; NULL returns to the library's own buffer.  The caller keeps ownership.
+ * ML_ERR_INVALID_ARG if dptr is not 4-byte-aligned device (or managed) memory of the context's
+ * device; the size cannot be checked and is the caller's responsibility. */
 int ml_use_device_map(ml_ctx *ctx, void *dptr);
 
 /* Launch on this CUDA stream (a cudaStream_t as void*, e.g. torch's current stream;

@@ -586,6 +586,16 @@ int ml_get_map_device(const ml_ctx *c, void **dptr)
 int ml_use_device_map(ml_ctx *c, void *dptr)
 {
     if (!c) return ML_ERR_INVALID_ARG;
+    if (dptr) { // must be device (or managed) memory of this context's device, 4-byte aligned; the size is the caller's word
+        cudaPointerAttributes a;
+        if (cudaPointerGetAttributes(&a, dptr) != cudaSuccess) {
+            cudaGetLastError();
+            return ML_ERR_INVALID_ARG;
+        }
+        if ((a.type != cudaMemoryTypeDevice && a.type != cudaMemoryTypeManaged) || a.device != c->device ||
+            (reinterpret_cast<uintptr_t>(dptr) & 3) != 0)
+            return ML_ERR_INVALID_ARG;
+    }
     c->map = dptr ? (unsigned int *)dptr : c->map_own;
     return ML_OK;
 }

@@ -198,5 +198,31 @@ def test_caller_owned_torch_map_and_stream():
         s.synchronize()
         assert np.array_equal(t.cpu().numpy().astype(np.uint32), ref)
         assert ml.ml_get_map_device(m.ctx) == t.data_ptr()
+        # host memory, or a misaligned device pointer, is refused and leaves the map in place
+        host = np.zeros(p.n_pix * p.n_pix, dtype=np.uint32)
+        for bad in (host.ctypes.data, t.data_ptr() + 2):
+            with pytest.raises(ml.MicrolensError) as e:
+                m.use_device_map(bad)
+            assert e.value.code == ml.ML_ERR_INVALID_ARG
+        assert ml.ml_get_map_device(m.ctx) == t.data_ptr()
         m.use_device_map(0)
+        # NULL = the legacy default stream: a shoot there is ordered after earlier work of every blocking stream, so a
+        # map zeroed / filled by torch on its own (blocking) stream right before is seen as written, while unrelated
+        # work keeps a second torch stream busy
+        m.use_device_map(t.data_ptr())
         m.attach_stream(0)
+        busy = torch.cuda.Stream()
+        with torch.cuda.stream(busy):
+            junk = torch.randn(4096, 4096, device="cuda:0")
+            for _ in range(4):
+                junk = junk @ junk
+                junk = junk / junk.abs().max()
+        t.fill_(123)                       # torch's current stream = legacy default stream here
+        m.shoot()                          # zeroes the map itself, then shoots, on the legacy stream
+        assert np.array_equal(t.cpu().numpy().astype(np.uint32), ref)
+        m.shoot_region(0, g.n1, 0, g.n2 // 2)
+        t2 = t.clone()                     # ordered after the shoot on the same legacy stream
+        m.shoot_region(0, g.n1, g.n2 // 2, g.n2, accumulate=True)
+        torch.cuda.synchronize()
+        assert np.array_equal(t.cpu().numpy().astype(np.uint32), ref) and int(t2.sum()) < int(t.sum())
+        m.use_device_map(0)

@@ -20,7 +20,10 @@
  *   ora_ray_x           BASELINE.json:configs[0] "regular grid over the rectangle";
  *                       PAPER.md:167 (regular grid).  Readings R7, R8.  ray_mode 1: GPU-D's random
  *                       ray positions, one per grid cell (reading R17), drawn
- *                       with Philox-4x32-10 keyed by the seed, counter = ray id.
+ *                       with Philox-4x32-10 keyed by the seed, counter = ray id.  ray_mode 2: the
+ *                       same draw spread over the WHOLE shooting rectangle -- every ray an independent
+ *                       uniform point of it, the literal reading of PAPER.md:131, :167 ("random
+ *                       positions in the shooting grid ... will introduce Poisson noise"; reading R20).
  *   ora_lens_equation   PAPER.md:49-54 eq.(4) with m_i = 1; the *_m variants take
  *                       the masses m_i of eq.(4).
  *   ora_pixel           PAPER.md:45-47 (rays "mapped to a grid of pixels in the
@@ -56,8 +59,9 @@ typedef struct {
     double n_rays;           /* mean rays per pixel without lensing */
     double L;                /* source-plane side length, Einstein radii */
     int32_t ray_mode;        /* 0: regular grid (configs); 1: random position inside
-                                each grid cell (the GPU-D way; reading R17)    */
-    uint64_t ray_seed;       /* key of the counter-based generator for ray_mode 1                  */
+                                each grid cell (the GPU-D way; reading R17);
+                                2: random position in the whole shooting rectangle (reading R20)   */
+    uint64_t ray_seed;       /* key of the counter-based generator for ray_modes 1 and 2           */
 } ora_problem;
 
 typedef struct {
@@ -86,7 +90,7 @@ int ora_derive(const ora_problem *p, ora_geometry *g)
     if (!p || !g) return ORA_BAD;
     if (!(p->sigma >= 0.0) || !(p->stellar_fraction >= 0.0) || !(p->stellar_fraction <= 1.0) ||
         p->n_pix <= 0 || !(p->n_rays > 0.0) || !(p->L > 0.0) || !isfinite(p->gamma) ||
-        !isfinite(p->sigma) || !isfinite(p->n_rays) || !isfinite(p->L) || (p->ray_mode != 0 && p->ray_mode != 1))
+        !isfinite(p->sigma) || !isfinite(p->n_rays) || !isfinite(p->L) || (p->ray_mode < 0 || p->ray_mode > 2))
         return ORA_BAD;
     double minus = 1.0 - p->sigma - p->gamma; /* axis-1 smooth stretch (eq.4, eq.11) */
     double plus = 1.0 - p->sigma + p->gamma;  /* axis-2 smooth stretch               */
@@ -144,9 +148,21 @@ void ora_ray_uniforms(uint64_t ray_id, uint64_t seed, double u[2])
  * origin (reading R7).  ray_mode 1: a uniformly random point of the same grid cell
  * [(i - n1/2) delta, (i + 1 - n1/2) delta) x [...]: the paper's GPU-D shoots rays "from random positions in
  * the shooting grid"; reading R17 keeps one ray per cell so that ray (i, j) stays
- * where the tile-local arithmetic and the region / sharding logic expect it (the regular grid is u = 1/2). */
+ * where the tile-local arithmetic and the region / sharding logic expect it (the regular grid is u = 1/2).
+ * ray_mode 2 (reading R20): the n1 n2 rays are independent uniform points of the whole rectangle
+ * [-n1 delta/2, n1 delta/2) x [-n2 delta/2, n2 delta/2) -- what "a batch of 2^17 random ray positions"
+ * "in the shooting grid" says literally; (i, j) only numbers the rays
+ * (id = j n1 + i is the counter), it says nothing about where the ray is.  Counts in any fixed area are then
+ * binomial ~ Poisson, the noise PAPER.md:167 describes. */
 static void ora_ray_x(const ora_problem *p, const ora_geometry *g, int64_t i, int64_t j, double x[2])
 {
+    if (p->ray_mode == 2) {
+        double u[2];
+        ora_ray_uniforms((uint64_t)j * (uint64_t)g->n1 + (uint64_t)i, p->ray_seed, u);
+        x[0] = (u[0] * (double)g->n1 - (double)g->n1 / 2.0) * g->delta;
+        x[1] = (u[1] * (double)g->n2 - (double)g->n2 / 2.0) * g->delta;
+        return;
+    }
     if (p->ray_mode == 1) {
         double u[2];
         ora_ray_uniforms((uint64_t)j * (uint64_t)g->n1 + (uint64_t)i, p->ray_seed, u);

@@ -97,10 +97,18 @@ def _load():
     return _lib
 
 
-def _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_seed=None):
-    """ray_seed = None: regular ray grid; an int: random position inside each grid cell (reading R17)."""
+RAY_MODES = {"regular": 0, "cell": 1, "uniform": 2}
+
+
+def _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_seed=None, ray_mode=None):
+    """ray_seed = None: regular ray grid; an int: random rays -- ray_mode "cell" (default): one random position inside
+    each grid cell (reading R17); "uniform": every ray an independent uniform point of the whole shooting rectangle
+    (reading R20, the literal GPU-D generation of PAPER.md:131, :167)."""
+    if ray_seed is None:
+        assert ray_mode in (None, "regular")
+        return _Problem(float(sigma), float(stellar_fraction), float(gamma), int(n_pix), float(n_rays), float(L), 0, 0)
     return _Problem(float(sigma), float(stellar_fraction), float(gamma), int(n_pix),
-                    float(n_rays), float(L), 0 if ray_seed is None else 1, 0 if ray_seed is None else int(ray_seed))
+                    float(n_rays), float(L), RAY_MODES[ray_mode or "cell"], int(ray_seed))
 
 
 def _dptr(a):
@@ -145,13 +153,13 @@ def geometry(sigma, stellar_fraction, gamma, n_pix, n_rays, L) -> Geometry:
 
 
 def shoot_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy,
-                 region=None, map_out=None, mass=None, ray_seed=None):
+                 region=None, map_out=None, mass=None, ray_seed=None, ray_mode=None):
     """Counts map (uint32, shape (n_pix, n_pix), [j', i']) and stats dict.
 
     region = (i0, i1, j0, j1) ray-index rectangle (default: the whole grid);
     map_out: existing map to accumulate into.
     """
-    p = _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_seed)
+    p = _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_seed, ray_mode)
     g = geometry(sigma, stellar_fraction, gamma, n_pix, n_rays, L)
     xy, n = _lenses(lens_xy)
     i0, i1, j0, j1 = region if region is not None else (0, g.n1, 0, g.n2)
@@ -172,13 +180,15 @@ def shoot_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy,
     return m, stats
 
 
-def shoot(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, mass=None, ray_seed=None):
-    return shoot_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, mass=mass, ray_seed=ray_seed)
+def shoot(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, mass=None, ray_seed=None, ray_mode=None):
+    return shoot_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, mass=mass, ray_seed=ray_seed,
+                        ray_mode=ray_mode)
 
 
-def capture_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, region, mass=None, ray_seed=None):
+def capture_region(sigma, stellar_fraction, gamma, n_pix, n_rays, L, lens_xy, region, mass=None, ray_seed=None,
+                   ray_mode=None):
     """y of every ray in region, shape (j1-j0, i1-i0, 2)."""
-    p = _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_seed)
+    p = _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_seed, ray_mode)
     xy, n = _lenses(lens_xy)
     i0, i1, j0, j1 = region
     out = np.empty((j1 - j0, i1 - i0, 2), dtype=np.float64)
@@ -243,9 +253,10 @@ def ray_uniforms(ray_id, seed):
     return float(u[0]), float(u[1])
 
 
-def ray_positions(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_i, ray_j, ray_seed=None):
-    """Image-plane positions x (n, 2) of the listed rays (regular grid, or random-in-cell with ray_seed)."""
-    p = _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_seed)
+def ray_positions(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_i, ray_j, ray_seed=None, ray_mode=None):
+    """Image-plane positions x (n, 2) of the listed rays (regular grid, or random with ray_seed: ray_mode "cell" /
+    "uniform")."""
+    p = _problem(sigma, stellar_fraction, gamma, n_pix, n_rays, L, ray_seed, ray_mode)
     ri = np.ascontiguousarray(ray_i, dtype=np.int64)
     rj = np.ascontiguousarray(ray_j, dtype=np.int64)
     out = np.empty((ri.size, 2), dtype=np.float64)

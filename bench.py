@@ -173,6 +173,9 @@ def config_dict(p, info, args):
         c["masses"] = "log-uniform 0.3-3 (workloads.lens_masses), eq. 4 with m_i"
     if getattr(args, "random_rays", False):
         c["ray_mode"] = "random position in every grid cell (GPU-D's ray generation, PAPER.md:131; reading R17), generic kernel"
+    if getattr(args, "uniform_rays", False):
+        c["ray_mode"] = ("every ray an independent uniform point of the shooting rectangle (the literal GPU-D ray generation, "
+                         "PAPER.md:131, :167; reading R20): bucket sort on the device + shoot_kernel_upipe, both inside the step")
     if getattr(args, "n_lenses", 0) > 0:
         c["n_lenses_override"] = "lens count set to %d in the same disk (large-N* row, not a BASELINE config)" % args.n_lenses
     if info is not None:
@@ -215,6 +218,8 @@ class ShootRig:
         self.m.set_lenses(self.xy, self.mass)
         if args.random_rays:
             self.m.set_ray_mode(ml.ML_RAYS_RANDOM, 20100527)
+        if args.uniform_rays:
+            self.m.set_ray_mode(ml.ML_RAYS_UNIFORM, 20100527)
         self.info = info = self.m.info
         self.n1, self.n2, self.n_lens = int(info["n1"]), int(info["n2"]), int(info["n_lenses"])
         self.j0, self.j1 = row_band(self.n2, rank, world, int(info["tile_h"]))
@@ -408,7 +413,7 @@ def run_ours(args):
     inter_per_launch = (rays_all // world) * n_lens / max(1, launches_all // max(world, 1))
     achieved = N_FLOP * inter_per_launch / kernel_s_per_launch / 1e12
     # ncu DRAM bytes exist only for the exact kernel that was captured: the BASELINE workload, unit masses, regular grid
-    plain = world == 1 and not (args.masses or args.random_rays or args.n_lenses > 0)
+    plain = world == 1 and not (args.masses or args.random_rays or args.uniform_rays or args.n_lenses > 0)
     traffic, traffic_src = NCU_DRAM_BYTES_PER_LAUNCH.get((p.name, args.precision), (None, None)) if plain else (None, None)
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved / peak_tflops, "traffic": traffic,
@@ -584,6 +589,8 @@ def main():
                     help="shoot = the hot path (default, the BASELINE.json metric); mapstats = the map-comparison row")
     ap.add_argument("--masses", action="store_true", help="unequal lens masses (eq. 4 with m_i): the MASS kernel instantiations")
     ap.add_argument("--random-rays", action="store_true", help="ML_RAYS_RANDOM: the paper's GPU-D ray generation")
+    ap.add_argument("--uniform-rays", action="store_true",
+                    help="ML_RAYS_UNIFORM: independent uniform ray positions over the whole rectangle (Poisson noise)")
     ap.add_argument("--n-lenses", type=int, default=0, help="override the lens count (large-N* row); 0 = eq. 5")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -76,7 +76,17 @@ enum {
  * (one reciprocal per interaction). */
 enum {
     ML_RAYS_REGULAR = 0,
-    ML_RAYS_RANDOM = 1
+    ML_RAYS_RANDOM = 1,
+    ML_RAYS_UNIFORM = 2  /* the literal reading of PAPER.md:131, :167 (reading R20): the n1 n2 rays are independent
+                            uniform points of the whole shooting rectangle,
+                                x = ((u1 n1 - n1/2) delta, (u2 n2 - n2/2) delta),  (u1, u2) drawn as above from ray id = j n1 + i,
+                            so the counts carry the Poisson noise the paper describes (ML_RAYS_RANDOM's one ray per cell is a
+                            stratified sample with less).  (i, j) only numbers the rays: a region of ml_shoot_region /
+                            ml_capture_region selects ray ids, not a patch of the image plane.  The library sorts the rays
+                            into buckets of 128 x 64 grid cells on the device (8 bytes of scratch per ray, kept by the context, up to
+                            45 % of the device memory; more rays are done in several passes) and shoots each bucket in
+                            coordinates local to it; ml_info.tile_w / tile_h report the bucket.  The lens loop is not split
+                            over CTAs in this mode. */
 };
 
 typedef struct {
@@ -96,7 +106,7 @@ typedef struct {
     int32_t sm_count;                /* multiProcessorCount of that device                  */
     int32_t sm_clock_khz;            /* cudaDevAttrClockRate (max SM clock)                 */
     int32_t ray_mode;                /* ML_RAYS_*                                           */
-    uint64_t ray_seed;               /* key of the ray generator (ML_RAYS_RANDOM)           */
+    uint64_t ray_seed;               /* key of the ray generator (ML_RAYS_RANDOM / _UNIFORM) */
 } ml_info;
 
 typedef struct {
@@ -144,7 +154,7 @@ int ml_set_lenses(ml_ctx *ctx, const double *xy, int64_t n);
  * non-positive mass; the previous lenses stay in place on any error. */
 int ml_set_lens_masses(ml_ctx *ctx, const double *xy, const double *mass, int64_t n);
 
-/* Select ML_RAYS_* (see the enum); seed keys the generator of ML_RAYS_RANDOM and is ignored otherwise.
+/* Select ML_RAYS_* (see the enum); seed keys the generator of ML_RAYS_RANDOM / ML_RAYS_UNIFORM and is ignored otherwise.
  * Takes effect at the next shoot / capture / probe.  ML_ERR_INVALID_ARG for any other mode. */
 int ml_set_ray_mode(ml_ctx *ctx, int mode, uint64_t seed);
 

@@ -18,6 +18,7 @@ from .binding import (  # noqa: F401
     ML_PREC_FP64,
     ML_RAYS_RANDOM,
     ML_RAYS_REGULAR,
+    ML_RAYS_UNIFORM,
     MicrolensError,
     library_path,
     load,

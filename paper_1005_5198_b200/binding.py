@@ -33,6 +33,7 @@ EXPORTS = (
 
 ML_RAYS_REGULAR = 0
 ML_RAYS_RANDOM = 1
+ML_RAYS_UNIFORM = 2
 
 ML_MEM_HOST = 0
 ML_MEM_DEVICE = 1

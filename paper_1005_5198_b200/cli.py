@@ -50,6 +50,8 @@ def main(argv=None) -> int:
     ap.add_argument("--seed", type=int, default=0, help="seed of the synthetic lens disk when --lenses is absent")
     ap.add_argument("--precision", default="fp32_tiled", choices=sorted(PRECISIONS))
     ap.add_argument("--random-rays", type=int, default=None, metavar="SEED", help="random ray positions (GPU-D's way)")
+    ap.add_argument("--uniform-rays", type=int, default=None, metavar="SEED",
+                    help="every ray an independent uniform point of the shooting rectangle (Poisson noise, PAPER.md:167)")
     ap.add_argument("--device", type=int, default=0)
     ap.add_argument("--out", help="write the uint32 counts to this .npy file")
     ap.add_argument("--pgm", help="write a greyscale picture of Delta m to this .pgm file (presentation only)")
@@ -65,6 +67,8 @@ def main(argv=None) -> int:
         m.set_lenses(xy, mass)
         if a.random_rays is not None:
             m.set_ray_mode(_b.ML_RAYS_RANDOM, a.random_rays)
+        if a.uniform_rays is not None:
+            m.set_ray_mode(_b.ML_RAYS_UNIFORM, a.uniform_rays)
         m.shoot()
         st, counts = m.stats, m.counts()
     mu_mean = float(counts.mean()) / a.n_rays

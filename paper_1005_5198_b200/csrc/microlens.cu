@@ -39,6 +39,12 @@ struct ml_ctx {
     int precision;
     int ray_mode;            // ML_RAYS_*
     unsigned long long ray_seed;
+    // ML_RAYS_UNIFORM scratch, grown on demand and kept: bucketed ray lists, fill counts (+ 1 word: their maximum)
+    unsigned long long *uni_list;
+    size_t uni_list_entries;
+    unsigned int *uni_fill;
+    size_t uni_fill_entries;
+    unsigned int *h_uni_max; // pinned
     ml_stats stats;
 };
 
@@ -62,7 +68,10 @@ struct DeviceGuard {
 struct Mode {
     int tw, th;
 };
-constexpr int RXF = 4, RYF = 4, KFF = 64;  // FP32_TILED (shoot_kernel_pipe) and FP32_COMPENSATED
+#ifndef ML_KFF
+#define ML_KFF 64
+#endif
+constexpr int RXF = 4, RYF = 4, KFF = ML_KFF;  // FP32_TILED (shoot_kernel_pipe) and FP32_COMPENSATED
 constexpr int WARPS_T = 4, SHARED_T = 4, MINB_T = 3; // FP32_TILED: 128-thread CTAs, 3 per SM, all rows share
 // source-order knobs of shoot_kernel_pipe (same arithmetic, different ptxas schedule), picked by a sweep of all 256
 // values on the B200: 44 = rows reversed in stage 1, pair B's 1/r^2 after pair A's accumulations, sy before sx
@@ -81,6 +90,7 @@ static_assert(kRandWarps == kWarps, "mode_of: the random-ray kernels use 256-thr
 
 Mode mode_of(int precision, int ray_mode)
 {
+    if (ray_mode == ML_RAYS_UNIFORM) return {kUniBW, kUniBH}; // the patch of the image plane one CTA's rays come from
     if (precision == ML_PREC_FP64) return {32 * RXD, kWarps * RYD};
     if (ray_mode == ML_RAYS_RANDOM) return {32 * RXR, kWarps * RYR};
     return {32 * RXF, WARPS_T * RYF};
@@ -150,6 +160,48 @@ template <bool CAPTURE> cudaError_t launch(int precision, int ray_mode, dim3 g, 
     return p.mass ? launch_m<CAPTURE, true>(precision, g, p, s) : launch_m<CAPTURE, false>(precision, g, p, s);
 }
 
+// uniformly random rays over the whole rectangle (reading R20): bucketed ray lists, one CTA per
+// kUniSlots entries; shoot_kernel_upipe in the FP32 modes, the generic kernel in fp64
+template <int KF, bool CAPTURE, bool MASS, bool NEWTON> cudaError_t launch_upipe(dim3 g, const ShootParams &p, cudaStream_t s)
+{
+    constexpr size_t smem = upipe_smem_bytes(MASS);
+    static bool opted_in = false;
+    if (!opted_in) {
+        const cudaError_t e = cudaFuncSetAttribute(shoot_kernel_upipe<KF, 4, CAPTURE, MASS, NEWTON>,
+                                                   cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        opted_in = true;
+    }
+    shoot_kernel_upipe<KF, 4, CAPTURE, MASS, NEWTON><<<g, kUniWarps * 32, smem, s>>>(p);
+    return cudaGetLastError();
+}
+
+// list entries one CTA takes: 128 threads x 8 rays (shoot_kernel_upipe), 256 x 8 (the generic kernel in fp64)
+unsigned int uniform_slots(int precision) { return precision == ML_PREC_FP64 ? kThreads * RXD * RYD : kUniWarps * 32 * 4 * kRandRY; }
+
+// g.y = the largest bucket fill; turned into list slices of the kernel's size here
+template <bool CAPTURE, bool MASS> cudaError_t launch_u(int precision, dim3 g, const ShootParams &p, cudaStream_t s)
+{
+    g.y = (g.y + uniform_slots(precision) - 1) / uniform_slots(precision);
+    switch (precision) {
+    case ML_PREC_FP64:
+        shoot_kernel<double, RXD, RYD, KFD, false, CAPTURE, MASS, true, true><<<g, kThreads, 0, s>>>(p);
+        return cudaGetLastError();
+    case ML_PREC_FP32_COMPENSATED:
+        return launch_upipe<KFCP, CAPTURE, MASS, true>(g, p, s);
+    default:
+        return launch_upipe<KFF, CAPTURE, MASS, false>(g, p, s);
+    }
+}
+
+__global__ void max_fill_kernel(const unsigned int *fill, long long n, unsigned int *out)
+{
+    unsigned int m = 0;
+    for (long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (long long)gridDim.x * blockDim.x) m = max(m, fill[k]);
+    m = __reduce_max_sync(0xffffffffu, m);
+    if ((threadIdx.x & 31) == 0 && m) atomicMax(out, m);
+}
+
 ShootParams base_params(const ml_ctx *c)
 {
     ShootParams p;
@@ -172,7 +224,87 @@ ShootParams base_params(const ml_ctx *c)
     p.counters = c->counters;
     p.n1 = c->n1;
     p.ray_seed = c->ray_seed;
+    p.n1d = (double)c->n1;
+    p.n2d = (double)c->n2;
     return p;
+}
+
+// ML_RAYS_UNIFORM: shoot (or capture) the rays behind handles 0 .. n_handles - 1 (p.list_w / p.probe_ids say which).
+// The image plane is cut into buckets of kUniBW x kUniBH grid cells; as many bucket rows as the list memory holds are
+// done per pass: zero the fill counts, scatter the handles (every pass draws every ray again and keeps those of its
+// rows), read back the largest fill (it sizes the grid; a fill above the capacity repeats the pass with more room),
+// shoot.  Events ev0 / ev1 bracket everything.  Does not synchronise after the last launch.
+int uniform_run(ml_ctx *c, ShootParams p, long long n_handles, bool capture, uint64_t *launches)
+{
+    const long long nbx = (c->n1 + kUniBW - 1) / kUniBW, nby = (c->n2 + kUniBH - 1) / kUniBH;
+    const double mean = (double)n_handles * (double)kUniBW * (double)kUniBH / ((double)c->n1 * (double)c->n2);
+    unsigned int cap = (unsigned int)std::min(4.0e9, std::ceil(mean + 6.0 * std::sqrt(mean) + 32.0));
+    if (cudaEventRecord(c->ev0, c->stream) != cudaSuccess) return ML_ERR_CUDA;
+    long long row0 = 0;
+    while (row0 < nby) {
+        cap = (cap + 3u) & ~3u;
+        // list memory: at most 45 % of the device (82 GB of a B200's 180: C2's 8.4e9 rays in one pass), and never more
+        // than what is already held plus what is free less 8 GiB
+        size_t free_b = 0, total_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return ML_ERR_CUDA;
+        const double budget = std::min(0.45 * (double)total_b, (double)c->uni_list_entries * 8.0 + (double)free_b - 8.0 * 1073741824.0);
+        long long rows = (long long)(budget / ((double)nbx * cap * 8.0));
+        rows = std::max<long long>(1, std::min(rows, nby - row0));
+        if ((double)rows * (double)nbx > 2.0e9) rows = std::max<long long>(1, (long long)(2.0e9 / (double)nbx));
+        const size_t n_b = (size_t)rows * (size_t)nbx, need = n_b * cap;
+        if (need > c->uni_list_entries) {
+            if (c->uni_list) cudaFree(c->uni_list);
+            c->uni_list = nullptr;
+            c->uni_list_entries = 0;
+            if (cudaMalloc(&c->uni_list, need * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); return ML_ERR_OOM; }
+            c->uni_list_entries = need;
+        }
+        if (n_b + 1 > c->uni_fill_entries) {
+            if (c->uni_fill) cudaFree(c->uni_fill);
+            c->uni_fill = nullptr;
+            c->uni_fill_entries = 0;
+            if (cudaMalloc(&c->uni_fill, (n_b + 1) * sizeof(unsigned int)) != cudaSuccess) { cudaGetLastError(); return ML_ERR_OOM; }
+            c->uni_fill_entries = n_b + 1;
+        }
+        p.ray_list = c->uni_list;
+        p.bucket_fill = c->uni_fill;
+        p.bucket_cap = cap;
+        p.bucket_nx = nbx;
+        p.bucket_row0 = row0;
+        ScatterParams q;
+        q.sp = p;
+        q.n_handles = n_handles;
+        q.bucket_row1 = row0 + rows;
+        q.fill = c->uni_fill;
+        q.list = c->uni_list;
+        const int sblocks = (int)std::min<long long>((n_handles + kScatterRun - 1) / kScatterRun, (long long)c->sm_count * 32);
+        const int mblocks = (int)std::min<long long>(((long long)n_b + 255) / 256, (long long)c->sm_count * 8);
+        if (cudaMemsetAsync(c->uni_fill, 0, (n_b + 1) * sizeof(unsigned int), c->stream) != cudaSuccess) return ML_ERR_CUDA;
+        uniform_scatter_kernel<<<sblocks, 256, 0, c->stream>>>(q);
+        max_fill_kernel<<<mblocks, 256, 0, c->stream>>>(c->uni_fill, (long long)n_b, c->uni_fill + n_b);
+        if (cudaGetLastError() != cudaSuccess ||
+            cudaMemcpyAsync(c->h_uni_max, c->uni_fill + n_b, sizeof(unsigned int), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+            cudaStreamSynchronize(c->stream) != cudaSuccess)
+            return ML_ERR_CUDA;
+        *launches += 2;
+        const unsigned int mx = *c->h_uni_max;
+        if (mx > cap) { // (6 sigma above the mean: about once in 1e9 buckets)
+            if (mx >= 0xfffffff0u) return ML_ERR_OOM;
+            cap = mx;
+            continue;
+        }
+        if (mx > 0) {
+            const dim3 grid((unsigned int)n_b, mx, 1); // (y: launch_u turns the largest fill into list slices)
+            cudaError_t e;
+            if (capture) e = p.mass ? launch_u<true, true>(c->precision, grid, p, c->stream) : launch_u<true, false>(c->precision, grid, p, c->stream);
+            else e = p.mass ? launch_u<false, true>(c->precision, grid, p, c->stream) : launch_u<false, false>(c->precision, grid, p, c->stream);
+            if (e != cudaSuccess) return ML_ERR_CUDA;
+            *launches += 1;
+        }
+        row0 += rows;
+    }
+    if (cudaEventRecord(c->ev1, c->stream) != cudaSuccess) return ML_ERR_CUDA;
+    return ML_OK;
 }
 
 // Second half of a split launch (see lens_range in shoot_kernel.cuh): add the partial sums of the lens ranges, then
@@ -288,6 +420,11 @@ int shoot_region_impl(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1,
         const Mode m = mode_of(c);
         ShootParams p = base_params(c);
         p.i0 = i0; p.i1 = i1; p.j0 = j0; p.j1 = j1;
+        if (c->ray_mode == ML_RAYS_UNIFORM) { // the region selects ray ids; where the rays are is the generator's business
+            p.list_w = i1 - i0;
+            const int rc = uniform_run(c, p, (i1 - i0) * (j1 - j0), false, &launches);
+            if (rc != ML_OK) return rc;
+        } else {
         const long long ti0 = i0 / m.tw, tj0 = j0 / m.th;
         const long long tiles_x = (i1 - 1) / m.tw - ti0 + 1, tiles_y = (j1 - 1) / m.th - tj0 + 1;
         int split_len = 0;
@@ -310,6 +447,7 @@ int shoot_region_impl(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1,
             }
         if (cudaEventRecord(c->ev1, c->stream) != cudaSuccess) return ML_ERR_CUDA;
         }
+        } // not ML_RAYS_UNIFORM
     }
     if (cudaMemcpyAsync(c->h_counters, c->counters, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
         cudaStreamSynchronize(c->stream) != cudaSuccess)
@@ -384,6 +522,34 @@ int capture_tiles(ml_ctx *c, const std::vector<long long> &tiles /* pairs */, Si
     return rc;
 }
 
+// ML_RAYS_UNIFORM: positions of the rays behind handles 0 .. n - 1 (region-relative indices, or entries of `ids`).
+int capture_uniform(ml_ctx *c, ShootParams p, long long n, const std::vector<long long> *ids, double *y_out)
+{
+    double2 *d_buf = nullptr;
+    long long *d_ids = nullptr;
+    int rc = ML_OK;
+    if (cudaMalloc(&d_buf, (size_t)n * sizeof(double2)) != cudaSuccess ||
+        (ids && cudaMalloc(&d_ids, (size_t)n * sizeof(long long)) != cudaSuccess)) {
+        cudaGetLastError();
+        rc = ML_ERR_OOM;
+    }
+    if (rc == ML_OK && ids &&
+        cudaMemcpyAsync(d_ids, ids->data(), (size_t)n * sizeof(long long), cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+        rc = ML_ERR_CUDA;
+    if (rc == ML_OK) {
+        p.capture = d_buf;
+        p.probe_ids = d_ids;
+        uint64_t launches = 0;
+        rc = uniform_run(c, p, n, true, &launches);
+    }
+    if (rc == ML_OK && (cudaMemcpyAsync(y_out, d_buf, (size_t)n * sizeof(double2), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
+                        cudaStreamSynchronize(c->stream) != cudaSuccess))
+        rc = ML_ERR_CUDA;
+    if (d_buf) cudaFree(d_buf);
+    if (d_ids) cudaFree(d_ids);
+    return rc;
+}
+
 } // namespace
 
 extern "C" {
@@ -446,7 +612,8 @@ int ml_create(double sigma, double stellar_fraction, double gamma, int32_t n_pix
         c->stream = c->own_stream;
         if (cudaMalloc(&c->map_own, (size_t)n_pix * n_pix * sizeof(unsigned int)) != cudaSuccess ||
             cudaMalloc(&c->counters, 3 * sizeof(unsigned long long)) != cudaSuccess ||
-            cudaMallocHost(&c->h_counters, 3 * sizeof(unsigned long long)) != cudaSuccess) {
+            cudaMallocHost(&c->h_counters, 3 * sizeof(unsigned long long)) != cudaSuccess ||
+            cudaMallocHost(&c->h_uni_max, sizeof(unsigned int)) != cudaSuccess) {
             cudaGetLastError();
             rc = ML_ERR_OOM;
         }
@@ -478,6 +645,9 @@ void ml_destroy(ml_ctx *c)
             if (c->mass) cudaFree(c->mass);
             if (c->counters) cudaFree(c->counters);
             if (c->h_counters) cudaFreeHost(c->h_counters);
+            if (c->h_uni_max) cudaFreeHost(c->h_uni_max);
+            if (c->uni_list) cudaFree(c->uni_list);
+            if (c->uni_fill) cudaFree(c->uni_fill);
             if (c->ev0) cudaEventDestroy(c->ev0);
             if (c->ev1) cudaEventDestroy(c->ev1);
             if (c->own_stream) cudaStreamDestroy(c->own_stream);
@@ -548,9 +718,9 @@ int ml_set_precision(ml_ctx *c, int mode)
 
 int ml_set_ray_mode(ml_ctx *c, int mode, uint64_t seed)
 {
-    if (!c || (mode != ML_RAYS_REGULAR && mode != ML_RAYS_RANDOM)) return ML_ERR_INVALID_ARG;
+    if (!c || (mode != ML_RAYS_REGULAR && mode != ML_RAYS_RANDOM && mode != ML_RAYS_UNIFORM)) return ML_ERR_INVALID_ARG;
     c->ray_mode = mode;
-    c->ray_seed = mode == ML_RAYS_RANDOM ? seed : 0;
+    c->ray_seed = mode == ML_RAYS_REGULAR ? 0 : seed;
     return ML_OK;
 }
 
@@ -624,6 +794,12 @@ int ml_capture_region(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1,
     if ((double)(i1 - i0) * (double)(j1 - j0) > 268435456.0) return ML_ERR_OOM;
     DeviceGuard g(c->device);
     if (!g.ok) return ML_ERR_CUDA;
+    if (c->ray_mode == ML_RAYS_UNIFORM) {
+        ShootParams p = base_params(c);
+        p.i0 = i0; p.i1 = i1; p.j0 = j0; p.j1 = j1;
+        p.list_w = i1 - i0;
+        return capture_uniform(c, p, (i1 - i0) * (j1 - j0), nullptr, y_out);
+    }
     const Mode m = mode_of(c);
     std::vector<long long> tiles;
     try {
@@ -666,6 +842,16 @@ int ml_probe(ml_ctx *c, int64_t n, const int64_t *ray_i, const int64_t *ray_j, d
         if (ray_i[k] < 0 || ray_i[k] >= c->n1 || ray_j[k] < 0 || ray_j[k] >= c->n2) return ML_ERR_INVALID_ARG;
     DeviceGuard g(c->device);
     if (!g.ok) return ML_ERR_CUDA;
+    if (c->ray_mode == ML_RAYS_UNIFORM) {
+        std::vector<long long> ids;
+        try {
+            ids.resize((size_t)n);
+        } catch (const std::bad_alloc &) {
+            return ML_ERR_OOM;
+        }
+        for (int64_t k = 0; k < n; ++k) ids[(size_t)k] = ray_j[k] * c->n1 + ray_i[k];
+        return capture_uniform(c, base_params(c), n, &ids, y_out);
+    }
     const Mode m = mode_of(c);
     // rays sorted by the tile that owns them; one capture tile per distinct tile
     std::vector<int64_t> order;

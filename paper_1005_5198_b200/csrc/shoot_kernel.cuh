@@ -58,6 +58,14 @@ struct ShootParams {
     double2 *partial;         // CAPTURE with split_len > 0: [gridDim.y][gridDim.x][TW*TH] partial sums (Sx, Sy)
     long long n1;             // rays per row of the whole grid (ray id = j*n1 + i, RANDOM instantiations)
     unsigned long long ray_seed; // key of the ray generator (RANDOM instantiations)
+    // ---- ML_RAYS_UNIFORM (shoot_kernel_upipe): rays sorted into buckets of kUniBW x kUniBH grid cells
+    const unsigned long long *ray_list; // [buckets of this launch][bucket_cap] ray handles (see uniform_ray_id)
+    const unsigned int *bucket_fill;    // [buckets of this launch] rays scattered into each bucket (may exceed bucket_cap)
+    unsigned int bucket_cap;
+    long long bucket_nx, bucket_row0;   // buckets per row of the bucket grid; bucket row of block x = 0
+    double n1d, n2d;                    // n1, n2 as doubles
+    long long list_w;                   // handle -> ray: width of the region the handles index (0 with probe_ids)
+    const long long *probe_ids;         // handle -> ray id by table (ml_probe); nullptr: handle = (j - j0) list_w + (i - i0)
 };
 
 constexpr int kThreads = 256;
@@ -119,9 +127,10 @@ __device__ __forceinline__ double fma_rn(double a, double b, double c) { return 
 // Philox-4x32-10 (Salmon et al., SC'11), counter = (ray id lo, hi, 0, 0), key = seed: two 53-bit uniforms in
 // [0,1) per ray.  GPU-D shoots rays from random positions; reading R17 draws one ray
 // uniformly inside each grid cell, so ray (i,j) stays in the tile that owns cell (i,j).
-__device__ __forceinline__ void ray_uniforms(unsigned long long ray_id, unsigned long long seed, double &u1, double &u2)
+__device__ __forceinline__ void ray_words(unsigned long long ray_id, unsigned long long seed, unsigned int &c0, unsigned int &c1,
+                                          unsigned int &c2, unsigned int &c3)
 {
-    unsigned int c0 = (unsigned int)ray_id, c1 = (unsigned int)(ray_id >> 32), c2 = 0u, c3 = 0u;
+    c0 = (unsigned int)ray_id; c1 = (unsigned int)(ray_id >> 32); c2 = 0u; c3 = 0u;
     unsigned int k0 = (unsigned int)seed, k1 = (unsigned int)(seed >> 32);
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
@@ -130,8 +139,26 @@ __device__ __forceinline__ void ray_uniforms(unsigned long long ray_id, unsigned
         c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
         k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
     }
+}
+
+__device__ __forceinline__ void ray_uniforms(unsigned long long ray_id, unsigned long long seed, double &u1, double &u2)
+{
+    unsigned int c0, c1, c2, c3;
+    ray_words(ray_id, seed, c0, c1, c2, c3);
     u1 = ((double)(c0 >> 5) * 67108864.0 + (double)(c1 >> 6)) * (1.0 / 9007199254740992.0);
     u2 = ((double)(c2 >> 5) * 67108864.0 + (double)(c3 >> 6)) * (1.0 / 9007199254740992.0);
+}
+
+// ML_RAYS_UNIFORM (see shoot_kernel_upipe below): bucket size and the ray a list entry stands for
+constexpr int kUniBW = 128, kUniBH = 64; // bucket: grid cells along axis 1 / axis 2 (the FP32 error of a close passage grows
+                                         // with the distance of ray and lens from the local origin: DESIGN.md R15)
+constexpr int kUniWarps = 4;             // shoot_kernel_upipe: 128 threads x 8 rays = 1024 list entries per CTA, 4 CTAs per SM
+
+__host__ __device__ __forceinline__ unsigned long long uniform_ray_id(const ShootParams &p, unsigned long long handle)
+{
+    if (p.probe_ids) return (unsigned long long)p.probe_ids[handle];
+    const long long jj = (long long)handle / p.list_w, ii = (long long)handle - jj * p.list_w;
+    return (unsigned long long)((p.j0 + jj) * p.n1 + (p.i0 + ii));
 }
 
 // a4 + a5 (+ statistics) for one thread's RX x RY rays: macro terms and pixel index in
@@ -144,10 +171,14 @@ __device__ __forceinline__ void ray_uniforms(unsigned long long ray_id, unsigned
 // field of u not all ones: F2I maps NaN to 0, so the test cannot be skipped).  CAPTURE writes y itself.
 // RANDOM instantiations either pass the (u1, u2) they drew in the prologue (UV_SMEM: shared memory, [ray][thread]) or
 // have them drawn again here (same counter, same key: the same numbers).
-template <int RX, int RY, bool CAPTURE, int WARPS = kWarps, bool RANDOM = false, bool UV_SMEM = false>
+// UNIFORM (ML_RAYS_UNIFORM, reading R20): slot (r, c) of thread t is entry (r RX + c) THREADS + t of the CTA's slice of a
+// bucket's ray list (`handles`, `n_valid` entries); the ray's position is x = ((u1 n1 - n1/2) delta, (u2 n2 - n2/2) delta)
+// with the uniforms of its ray id, kept in `uv`.  CAPTURE writes y to capture[handle].
+template <int RX, int RY, bool CAPTURE, int WARPS = kWarps, bool RANDOM = false, bool UV_SMEM = false, bool UNIFORM = false>
 __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, long long tj, long long t, int lane,
                                             int warp, const double (&Sx)[RY][RX], const double (&Sy)[RY][RX],
-                                            unsigned int *cta_count, const double2 *uv = nullptr)
+                                            unsigned int *cta_count, const double2 *uv = nullptr, int n_valid = 0,
+                                            const unsigned long long *handles = nullptr)
 {
     constexpr int TW = 32 * RX;
     constexpr int TH = WARPS * RY;
@@ -174,6 +205,20 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
 #pragma unroll
             for (int c = 0; c < RX; ++c) {
                 double x1, x2;
+                if (UNIFORM) {
+                    const int slot = (r * RX + c) * THREADS + (int)threadIdx.x;
+                    if (slot >= n_valid) continue;
+                    double2 w;
+                    if (UV_SMEM) w = uv[slot];
+                    else ray_uniforms(uniform_ray_id(p, handles[slot]), p.ray_seed, w.x, w.y);
+                    x1 = __dmul_rn(__dsub_rn(__dmul_rn(w.x, p.n1d), 0.5 * p.n1d), p.delta);
+                    x2 = __dmul_rn(__dsub_rn(__dmul_rn(w.y, p.n2d), 0.5 * p.n2d), p.delta);
+                    const double y1 = p.c1 * x1 - Sx[r][c], y2 = p.c2 * x2 - Sy[r][c];
+                    const bool finite = (fabs(y1) <= 1.7976931348623157e308) && (fabs(y2) <= 1.7976931348623157e308);
+                    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+                    p.capture[handles[slot]] = make_double2(finite ? y1 : qnan, finite ? y2 : qnan);
+                    continue;
+                }
                 if (RANDOM) { // the ray's own position in its cell (the draw of the prologue)
                     const double2 w = draw(r, c);
                     x1 = ((ib + (double)c) + w.x - (p.half1 + 0.5)) * p.delta;
@@ -208,6 +253,7 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
         const long long j = tj * TH + warp * RY + r;
         rowmask |= ((j >= p.j0) && (j < p.j1)) ? (1u << r) : 0u;
     }
+    if (UNIFORM) { colmask = 0xffffffffu; rowmask = 0xffffffffu; } // every listed ray belongs to the region: slots decide
     const unsigned int n_pix_u = (unsigned int)p.n_pix;
     const double nip = -p.inv_pixel;
 #pragma unroll
@@ -217,7 +263,16 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
 #pragma unroll
         for (int c = 0; c < RX; ++c) {
             double b1, b2;
-            if (RANDOM) {
+            bool in_list = true;
+            if (UNIFORM) {
+                const int slot = (r * RX + c) * THREADS + (int)threadIdx.x;
+                in_list = slot < n_valid;
+                double2 w = make_double2(0.5, 0.5);
+                if (UV_SMEM) w = uv[slot];
+                else if (in_list) ray_uniforms(uniform_ray_id(p, handles[slot]), p.ray_seed, w.x, w.y);
+                b1 = __fma_rn(__dmul_rn(__dsub_rn(__dmul_rn(w.x, p.n1d), 0.5 * p.n1d), p.delta), p.k1, p.hoff);
+                b2 = __fma_rn(__dmul_rn(__dsub_rn(__dmul_rn(w.y, p.n2d), 0.5 * p.n2d), p.delta), p.k2, p.hoff);
+            } else if (RANDOM) {
                 const double2 w = draw(r, c);
                 b1 = __fma_rn(((ib + (double)c) + w.x - (p.half1 + 0.5)) * p.delta, p.k1, p.hoff);
                 b2 = __fma_rn(((jb + (double)r) + w.y - (p.half2 + 0.5)) * p.delta, p.k2, p.hoff);
@@ -229,7 +284,7 @@ __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, 
             const double u2 = __fma_rn(Sy[r][c], nip, b2);
             // finite <=> exponent field not all ones, in both components
             const bool finite = ((~__double2hiint(u1) & 0x7ff00000) != 0) && ((~__double2hiint(u2) & 0x7ff00000) != 0);
-            const bool valid = ((colmask >> c) & (rowmask >> r) & 1u) != 0u;
+            const bool valid = UNIFORM ? in_list : (((colmask >> c) & (rowmask >> r) & 1u) != 0u);
             // floor to int (saturating): 0 <= u < n_pix  <=>  (unsigned)floor(u) < n_pix for every finite u
             const int pi = __double2int_rd(u1), pj = __double2int_rd(u2);
             const bool inside = ((unsigned int)pi < n_pix_u) && ((unsigned int)pj < n_pix_u);
@@ -337,9 +392,11 @@ __global__ void __launch_bounds__(WARPS * 32) combine_kernel(const ShootParams p
     finish_tile<RX, RY, CAPTURE, WARPS, RANDOM, false>(p, ti, tj, t, lane, warp, Sx, Sy, cta_count);
 }
 
-template <typename Real, int RX, int RY, int KF, bool NEWTON, bool CAPTURE, bool MASS = false, bool RANDOM = false>
+template <typename Real, int RX, int RY, int KF, bool NEWTON, bool CAPTURE, bool MASS = false, bool RANDOM = false, bool UNIFORM = false>
 __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
 {
+    static_assert(!UNIFORM || RANDOM, "UNIFORM: per-ray offsets");
+    constexpr int SLOTS = kThreads * RX * RY; // UNIFORM: list entries per CTA
     using Real2 = typename Vec2<Real>::type;
     constexpr int TW = 32 * RX;
     constexpr int TH = kWarps * RY;
@@ -354,16 +411,32 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
 
-    // ---- a6: which tile
-    long long t, ti, tj;
-    which_tile<CAPTURE>(p, t, ti, tj);
+    // ---- a6: which tile (UNIFORM: which slice of which bucket's ray list, as in shoot_kernel_upipe)
+    long long t = 0, ti = 0, tj = 0;
     int lb, le; // this CTA's lens range: [0, n_lens) except in split capture launches
-    lens_range<CAPTURE>(p, lb, le);
+    int n_valid = 0;
+    const unsigned long long *handles = nullptr;
+    double cx, cy, ccx = 0.0, ccy = 0.0;
+    if (UNIFORM) {
+        const long long b = (long long)blockIdx.x;
+        const unsigned int filled = min(p.bucket_fill[b], p.bucket_cap);
+        const long long first = (long long)blockIdx.y * SLOTS;
+        if (first >= (long long)filled) return; // (whole CTA: before any barrier)
+        n_valid = (int)min((long long)SLOTS, (long long)filled - first);
+        handles = p.ray_list + (size_t)b * p.bucket_cap + first;
+        lens_range<false>(p, lb, le);
+        ccx = (double)((b % p.bucket_nx) * kUniBW) + 0.5 * kUniBW;
+        ccy = (double)((p.bucket_row0 + b / p.bucket_nx) * kUniBH) + 0.5 * kUniBH;
+        cx = (ccx - 0.5 * p.n1d) * p.delta;
+        cy = (ccy - 0.5 * p.n2d) * p.delta;
+    } else {
+        which_tile<CAPTURE>(p, t, ti, tj);
+        lens_range<CAPTURE>(p, lb, le);
+        // ---- a2: tile centre (fp64) and this thread's ray offsets from it
+        cx = ((double)(ti * TW) + 0.5 * (TW - 1) - p.half1) * p.delta;
+        cy = ((double)(tj * TH) + 0.5 * (TH - 1) - p.half2) * p.delta;
+    }
     if (threadIdx.x < 3) cta_count[threadIdx.x] = 0;
-
-    // ---- a2: tile centre (fp64) and this thread's ray offsets from it
-    const double cx = ((double)(ti * TW) + 0.5 * (TW - 1) - p.half1) * p.delta;
-    const double cy = ((double)(tj * TH) + 0.5 * (TH - 1) - p.half2) * p.delta;
     Real ox[RX], oy[RY];
 #pragma unroll
     for (int c = 0; c < RX; ++c) ox[c] = (Real)(((double)(lane * RX + c) - 0.5 * (TW - 1)) * p.delta);
@@ -376,8 +449,20 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
         for (int r = 0; r < RY; ++r)
 #pragma unroll
             for (int c = 0; c < RX; ++c) {
-                const unsigned long long i = (unsigned long long)(ti * TW + lane * RX + c), j = (unsigned long long)(tj * TH + warp * RY + r);
                 double u1, u2;
+                if (UNIFORM) { // an empty slot shoots a ray from the bucket centre and throws it away
+                    const int slot = (r * RX + c) * kThreads + (int)threadIdx.x;
+                    Real fx = (Real)0, fy = (Real)0;
+                    if (slot < n_valid) {
+                        ray_uniforms(uniform_ray_id(p, handles[slot]), p.ray_seed, u1, u2);
+                        fx = (Real)((__dmul_rn(u1, p.n1d) - ccx) * p.delta);
+                        fy = (Real)((__dmul_rn(u2, p.n2d) - ccy) * p.delta);
+                    }
+                    oxr[RANDOM ? r : 0][RANDOM ? c : 0] = fx;
+                    oyr[RANDOM ? r : 0][RANDOM ? c : 0] = fy;
+                    continue;
+                }
+                const unsigned long long i = (unsigned long long)(ti * TW + lane * RX + c), j = (unsigned long long)(tj * TH + warp * RY + r);
                 ray_uniforms(j * (unsigned long long)p.n1 + i, p.ray_seed, u1, u2);
                 oxr[RANDOM ? r : 0][RANDOM ? c : 0] = (Real)(((double)(lane * RX + c) + u1 - 0.5 * TW) * p.delta);
                 oyr[RANDOM ? r : 0][RANDOM ? c : 0] = (Real)(((double)(warp * RY + r) + u2 - 0.5 * TH) * p.delta);
@@ -490,6 +575,10 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
         buf ^= 1;
     }
 
+    if (UNIFORM) {
+        finish_tile<RX, RY, CAPTURE, kWarps, true, false, true>(p, 0, 0, 0, lane, warp, Sx, Sy, cta_count, nullptr, n_valid, handles);
+        return;
+    }
     if (CAPTURE && p.partial) { store_partials<RX, RY, kWarps>(p, t, lane, warp, Sx, Sy); return; }
     finish_tile<RX, RY, CAPTURE, kWarps, RANDOM>(p, ti, tj, t, lane, warp, Sx, Sy, cta_count);
 }
@@ -999,6 +1088,269 @@ __global__ void __launch_bounds__(kRandWarps * 32, MINB) shoot_kernel_rpipe(cons
     }
     if (CAPTURE && p.partial) { store_partials<RX, RY, WARPS>(p, t, lane, warp, Sx, Sy); return; }
     finish_tile<RX, RY, CAPTURE, WARPS, true, true>(p, ti, tj, t, lane, warp, Sx, Sy, cta_count, uv_s);
+}
+
+// ---------------------------------------------------------------------------------------
+// Uniformly random ray positions over the whole shooting rectangle (ML_RAYS_UNIFORM: the literal GPU-D ray
+// generation, "a batch of 2^17 random ray positions" PAPER.md:131, "shot from random positions in the shooting grid ...
+// This will introduce Poisson noise" PAPER.md:167; reading R20).
+//
+// Ray id = j n1 + i only numbers the rays: its position is ((u1 n1 - n1/2) delta, (u2 n2 - n2/2) delta) with the two
+// uniforms of Philox-4x32-10(counter = id, key = seed).  FP32 terms need coordinates local to a small patch of the image
+// plane, so the rays are first sorted by position: uniform_scatter_kernel draws every ray of the requested id range and
+// appends its handle to the list of the bucket (kUniBW x kUniBH grid cells) it falls in; shoot_kernel_upipe then shoots
+// one CTA per 1024 list entries with the bucket centre as the local origin.  The list order depends on the order of the
+// atomics, the results do not: the arithmetic of a ray involves no other ray.  That is why the shared reciprocal pairs two
+// LENSES of one ray here, R = 1/(r2_k r2_k+1), 1/r2_k = R r2_k+1, 1/r2_k+1 = R r2_k (k even), not two rays of one lens as
+// in the kernels above; every second lens pair takes its own reciprocals instead (4 MUFU, no FMUL2: the XU pipe has room,
+// the FMA pipe is the bound), for every ray alike.  A thread owns 8 list entries as two "rows" of two packed pairs;
+// per row and lens pair: 8 FADD2, 8 FFMA2 (r^2), 3 FMUL2 + 2 x 2 MUFU (or 8 MUFU), 8 FFMA2: the instruction mix of
+// shoot_kernel_rpipe.  Lenses are added in index order, FP32 partial sums over KF lenses, fp64 accumulators, as everywhere.
+struct ScatterParams {
+    ShootParams sp;        // i0, j0, n1, n1d, n2d, ray_seed, list_w, probe_ids, bucket_nx, bucket_row0, bucket_cap
+    long long n_handles;   // rays to scatter: handles 0 .. n_handles - 1
+    long long bucket_row1; // bucket rows [bucket_row0, bucket_row1) are kept by this pass
+    unsigned int *fill;    // [rows x bucket_nx], zeroed by the caller
+    unsigned long long *list;
+};
+
+// Each block takes runs of kScatterRun consecutive handles; a thread steps through its run 256 handles at a time and
+// carries (row, column) of the region along, so the handle -> ray id division happens once per run.  The bucket is
+// taken from the integer part of u n (u as the 64-bit fraction c0:c1 / 2^64): within 1e-10 of a grid cell of the
+// double-precision position the shoot kernel uses -- a ray that close to a bucket edge may sit in either bucket.
+constexpr int kScatterRun = 256 * 16;
+__global__ void __launch_bounds__(256) uniform_scatter_kernel(const ScatterParams q)
+{
+    const unsigned long long n1 = (unsigned long long)q.sp.n1, n2 = (unsigned long long)q.sp.n2d;
+    for (long long run = (long long)blockIdx.x * kScatterRun; run < q.n_handles; run += (long long)gridDim.x * kScatterRun) {
+        long long h = run + threadIdx.x;
+        const long long end = min(run + (long long)kScatterRun, q.n_handles);
+        long long jj = 0, ii = 0;
+        if (!q.sp.probe_ids && h < end) { jj = h / q.sp.list_w; ii = h - jj * q.sp.list_w; }
+        for (; h < end; h += 256) {
+            const unsigned long long id = q.sp.probe_ids ? (unsigned long long)q.sp.probe_ids[h]
+                                                         : (unsigned long long)((q.sp.j0 + jj) * q.sp.n1 + (q.sp.i0 + ii));
+            unsigned int c0, c1, c2, c3;
+            ray_words(id, q.sp.ray_seed, c0, c1, c2, c3);
+            const long long bx = (long long)(__umul64hi(((unsigned long long)c0 << 32) | c1, n1) / kUniBW);
+            const long long by = (long long)(__umul64hi(((unsigned long long)c2 << 32) | c3, n2) / kUniBH);
+            if (by >= q.sp.bucket_row0 && by < q.bucket_row1) {
+                const long long b = (by - q.sp.bucket_row0) * q.sp.bucket_nx + bx;
+                const unsigned int slot = atomicAdd(&q.fill[b], 1u);
+                if (slot < q.sp.bucket_cap) q.list[(size_t)b * q.sp.bucket_cap + slot] = (unsigned long long)h;
+            }
+            ii += 256;
+            while (ii >= q.sp.list_w && !q.sp.probe_ids) { ii -= q.sp.list_w; ++jj; }
+        }
+    }
+}
+
+template <int RY> struct UPipeRegs {   // one row of a thread (two packed ray pairs A, B) x one lens pair (lenses 0, 1)
+    float m[2];
+    float2 dx[2][2], dy[2][2]; // [lens][ray pair]
+    float2 r2[2][2];           // r^2; own-reciprocal pairs: 1/r^2
+    float2 R[2];               // shared pairs: 1/(r2[0] r2[1]) per ray pair
+};
+
+template <int KF, int MINB, bool CAPTURE, bool MASS = false, bool NEWTON = false>
+__global__ void __launch_bounds__(kUniWarps * 32, MINB) shoot_kernel_upipe(const ShootParams p)
+{
+    constexpr int RX = 4, RY = kRandRY, WARPS = kUniWarps;
+    constexpr int THREADS = WARPS * 32;
+    constexpr int SLOTS = THREADS * RX * RY; // list entries per CTA
+    static_assert(kChunk % KF == 0 && KF % 4 == 0, "flush groups must tile a chunk in double lens pairs");
+    static_assert(RY == 2, "two rows per thread");
+    constexpr int PER_THREAD = kChunk / THREADS;
+
+    extern __shared__ __align__(16) unsigned char rp_smem[];
+    float4 *lens_s = reinterpret_cast<float4 *>(rp_smem);                                      // [2][kChunk + 4]
+    double2 *uv_s = reinterpret_cast<double2 *>(rp_smem + 2 * (kChunk + 4) * sizeof(float4)); // [RX*RY][THREADS]
+    float *mass_s = reinterpret_cast<float *>(rp_smem + 2 * (kChunk + 4) * sizeof(float4) +
+                                              (size_t)RX * RY * THREADS * sizeof(double2));   // [2][kChunk + 4]
+    __shared__ unsigned int cta_count[3];
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    // ---- which slice of which bucket list
+    const long long b = (long long)blockIdx.x;
+    const unsigned int filled = min(p.bucket_fill[b], p.bucket_cap);
+    const long long first = (long long)blockIdx.y * SLOTS;
+    if (first >= (long long)filled) return; // (whole CTA: before any barrier)
+    const int n_valid = (int)min((long long)SLOTS, (long long)filled - first);
+    const unsigned long long *handles = p.ray_list + (size_t)b * p.bucket_cap + first;
+    int lb, le;
+    lens_range<false>(p, lb, le);
+    if (threadIdx.x < 3) cta_count[threadIdx.x] = 0;
+    const float padc = -1e9f; // a padding lens must keep the shared product finite (see shoot_kernel_pipe, NEWTON)
+    if (threadIdx.x < 8) lens_s[(threadIdx.x >> 2) * (kChunk + 4) + kChunk + (threadIdx.x & 3)] = make_float4(padc, padc, padc, padc);
+    if (MASS && threadIdx.x < 8) mass_s[(threadIdx.x >> 2) * (kChunk + 4) + kChunk + (threadIdx.x & 3)] = 0.f;
+
+    // ---- a2: bucket centre (grid cells, fp64) and every listed ray's offset from it
+    const long long bxi = b % p.bucket_nx, byi = p.bucket_row0 + b / p.bucket_nx;
+    const double ccx = (double)(bxi * kUniBW) + 0.5 * kUniBW, ccy = (double)(byi * kUniBH) + 0.5 * kUniBH;
+    const double cx = (ccx - 0.5 * p.n1d) * p.delta, cy = (ccy - 0.5 * p.n2d) * p.delta;
+    float2 oxA[RY], oxB[RY], oyA[RY], oyB[RY];
+#pragma unroll
+    for (int r = 0; r < RY; ++r) {
+        float ox[RX], oy[RX];
+#pragma unroll
+        for (int c = 0; c < RX; ++c) {
+            const int slot = (r * RX + c) * THREADS + (int)threadIdx.x;
+            double2 w = make_double2(0.5, 0.5);
+            ox[c] = 0.f; oy[c] = 0.f; // an empty slot shoots a ray from the bucket centre and throws it away
+            if (slot < n_valid) {
+                ray_uniforms(uniform_ray_id(p, handles[slot]), p.ray_seed, w.x, w.y);
+                ox[c] = (float)((__dmul_rn(w.x, p.n1d) - ccx) * p.delta);
+                oy[c] = (float)((__dmul_rn(w.y, p.n2d) - ccy) * p.delta);
+            }
+            uv_s[slot] = w;
+        }
+        oxA[r] = make_float2(ox[0], ox[1]); oxB[r] = make_float2(ox[2], ox[3]);
+        oyA[r] = make_float2(oy[0], oy[1]); oyB[r] = make_float2(oy[2], oy[3]);
+    }
+
+    double Sx[RY][RX], Sy[RY][RX];
+    float2 sxA[RY], sxB[RY], syA[RY], syB[RY];
+#pragma unroll
+    for (int r = 0; r < RY; ++r) {
+#pragma unroll
+        for (int c = 0; c < RX; ++c) { Sx[r][c] = 0.0; Sy[r][c] = 0.0; }
+        sxA[r] = make_float2(0.f, 0.f); sxB[r] = sxA[r]; syA[r] = sxA[r]; syB[r] = sxA[r];
+    }
+
+    // ---- a1: lens staging (as in shoot_kernel_pipe)
+    double2 pre[PER_THREAD];
+    double pre_m[MASS ? PER_THREAD : 1];
+    auto fetch = [&](int base) {
+#pragma unroll
+        for (int q = 0; q < PER_THREAD; ++q) {
+            const int k = base + q * THREADS + threadIdx.x;
+            if (k < le) {
+                pre[q] = __ldg(&p.lens[k]);
+                if (MASS) pre_m[q] = __ldg(&p.mass[k]);
+            }
+        }
+    };
+    auto stage = [&](int base, int buf) {
+#pragma unroll
+        for (int q = 0; q < PER_THREAD; ++q) {
+            const int k = base + q * THREADS + threadIdx.x;
+            float nx = padc, ny = padc, m = 0.f;
+            if (k < le) {
+                nx = -(float)(pre[q].x - cx);
+                ny = -(float)(pre[q].y - cy);
+                if (MASS) m = (float)pre_m[q];
+            }
+            lens_s[buf * (kChunk + 4) + q * THREADS + threadIdx.x] = make_float4(nx, nx, ny, ny);
+            if (MASS) mass_s[buf * (kChunk + 4) + q * THREADS + threadIdx.x] = m;
+        }
+    };
+    fetch(lb);
+    stage(lb, 0);
+    __syncthreads();
+
+    // ---- a3: all-pairs deflection sum, two lenses at a time
+    const float2 eps2 = make_float2(0x1p-80f, 0x1p-80f);
+    auto newton = [](float2 a, float2 R) { // one Newton-Raphson step: R <- R + R (1 - a R)
+        const float2 e = __ffma2_rn(make_float2(-a.x, -a.y), R, make_float2(1.f, 1.f));
+        return __ffma2_rn(R, e, R);
+    };
+    // stage 1 of (row r, lens pair l0 l1): differences, r^2, reciprocals (own: of each r^2; shared: of the products)
+    auto stage1 = [&](auto own, int r, const float4 l0, const float4 l1, const float m0, const float m1, UPipeRegs<RY> &s) {
+        s.m[0] = m0; s.m[1] = m1;
+#pragma unroll
+        for (int L = 0; L < 2; ++L) {
+            const float4 l = L ? l1 : l0;
+            const float2 nlx = make_float2(l.x, l.y), nly = make_float2(l.z, l.w);
+            s.dx[L][0] = __fadd2_rn(oxA[r], nlx); s.dx[L][1] = __fadd2_rn(oxB[r], nlx);
+            s.dy[L][0] = __fadd2_rn(oyA[r], nly); s.dy[L][1] = __fadd2_rn(oyB[r], nly);
+#pragma unroll
+            for (int X = 0; X < 2; ++X) s.r2[L][X] = __ffma2_rn(s.dy[L][X], s.dy[L][X], __ffma2_rn(s.dx[L][X], s.dx[L][X], eps2));
+        }
+#pragma unroll
+        for (int X = 0; X < 2; ++X) {
+            if (decltype(own)::value) {
+#pragma unroll
+                for (int L = 0; L < 2; ++L) {
+                    float2 i;
+                    i.x = rcp_approx(s.r2[L][X].x); i.y = rcp_approx(s.r2[L][X].y);
+                    if (NEWTON) i = newton(s.r2[L][X], i);
+                    s.r2[L][X] = i;
+                }
+            } else {
+                const float2 P = __fmul2_rn(s.r2[0][X], s.r2[1][X]);
+                s.R[X].x = rcp_approx(P.x); s.R[X].y = rcp_approx(P.y);
+            }
+        }
+    };
+    // stage 2: 1/r^2 of both lenses and the accumulations, lens 0 before lens 1 (index order)
+    auto stage2 = [&](auto own, int r, const UPipeRegs<RY> &s) {
+#pragma unroll
+        for (int X = 0; X < 2; ++X) {
+            float2 i0, i1;
+            if (decltype(own)::value) {
+                i0 = s.r2[0][X]; i1 = s.r2[1][X];
+            } else {
+                float2 R = s.R[X];
+                if (NEWTON) R = newton(__fmul2_rn(s.r2[0][X], s.r2[1][X]), R);
+                i0 = __fmul2_rn(R, s.r2[1][X]);
+                i1 = __fmul2_rn(R, s.r2[0][X]);
+            }
+            if (MASS) { i0 = __fmul2_rn(i0, make_float2(s.m[0], s.m[0])); i1 = __fmul2_rn(i1, make_float2(s.m[1], s.m[1])); }
+            float2 &sx = X ? sxB[r] : sxA[r], &sy = X ? syB[r] : syA[r];
+            sx = __ffma2_rn(s.dx[0][X], i0, sx);
+            sy = __ffma2_rn(s.dy[0][X], i0, sy);
+            sx = __ffma2_rn(s.dx[1][X], i1, sx);
+            sy = __ffma2_rn(s.dy[1][X], i1, sy);
+        }
+    };
+
+    int buf = 0;
+    for (int base = lb; base < le; base += kChunk) {
+        const bool more = base + kChunk < le;
+        if (more) fetch(base + kChunk);
+        const int cnt = min(kChunk, le - base);
+        const int cntp = (cnt + 3) & ~3; // whole double pairs: up to three padding lenses at the very end
+        const float4 *ls = lens_s + buf * (kChunk + 4);
+        const float *ms = mass_s + buf * (kChunk + 4);
+        auto mass_of = [&](int k) { return MASS ? ms[k] : 1.f; };
+        UPipeRegs<RY> a, c;
+        const std::integral_constant<bool, false> shared;
+        const std::integral_constant<bool, true> own;
+        stage1(shared, 0, ls[0], ls[1], mass_of(0), mass_of(1), a);
+        for (int k0 = 0; k0 < cntp; k0 += KF) {
+            const int kend = min(k0 + KF, cntp);
+#pragma unroll 1
+            for (int k = k0; k < kend; k += 4) { // lens pairs (k, k+1): shared reciprocals; (k+2, k+3): own
+                stage1(shared, 1, ls[k], ls[k + 1], mass_of(k), mass_of(k + 1), c);
+                stage2(shared, 0, a);
+                stage1(own, 0, ls[k + 2], ls[k + 3], mass_of(k + 2), mass_of(k + 3), a);
+                stage2(shared, 1, c);
+                stage1(own, 1, ls[k + 2], ls[k + 3], mass_of(k + 2), mass_of(k + 3), c);
+                stage2(own, 0, a);
+                stage1(shared, 0, ls[k + 4], ls[k + 5], mass_of(k + 4), mass_of(k + 5), a); // (<= cntp + 1 <= kChunk + 3)
+                stage2(own, 1, c);
+            }
+#pragma unroll
+            for (int r = 0; r < RY; ++r) {
+                Sx[r][0] += (double)sxA[r].x; Sx[r][1] += (double)sxA[r].y;
+                Sx[r][2] += (double)sxB[r].x; Sx[r][3] += (double)sxB[r].y;
+                Sy[r][0] += (double)syA[r].x; Sy[r][1] += (double)syA[r].y;
+                Sy[r][2] += (double)syB[r].x; Sy[r][3] += (double)syB[r].y;
+                sxA[r] = make_float2(0.f, 0.f); sxB[r] = sxA[r]; syA[r] = sxA[r]; syB[r] = sxA[r];
+            }
+        }
+        if (more) stage(base + kChunk, buf ^ 1);
+        __syncthreads();
+        buf ^= 1;
+    }
+    finish_tile<RX, RY, CAPTURE, WARPS, true, true, true>(p, 0, 0, 0, lane, warp, Sx, Sy, cta_count, uv_s, n_valid, handles);
+}
+
+constexpr size_t upipe_smem_bytes(bool mass)
+{
+    return 2 * (kChunk + 4) * sizeof(float4) + (size_t)4 * kRandRY * kUniWarps * 32 * sizeof(double2) +
+           (mass ? 2 * (kChunk + 4) * sizeof(float) : 0);
 }
 
 } // namespace mlb200

@@ -17,8 +17,8 @@ import paper_1005_5198_b200 as ml
 from oracle import oracle
 from workloads import CONFIGS, lens_disk, probe_rays
 
-from parity_common import (PREC_NAME, check_maps, check_rays, make_pair, problem_args, report, run_subregions,
-                           subregion_tiles)
+from parity_common import (PREC_NAME, check_maps, check_rays, close_passage_share, make_pair, problem_args, report,
+                           run_subregions, subregion_tiles)
 
 pytestmark = pytest.mark.gpu
 
@@ -65,6 +65,24 @@ def test_subregions_all_four_criteria(cfg, precision):
         r = run_subregions(p, m, g, xy, tiles, precision)
         assert r["rays"] >= 4000000 or len(tiles) < 16
         report("%s sub-regions %s" % (p.name, PREC_NAME[precision]), r)
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4], ids=["C3", "C4", "C5"])
+def test_representative_ray_sample(cfg):
+    """The sub-rectangles above are sixteen patches of the image plane: they hold a lens or they do not.  Here 250 000
+    rays are drawn uniformly over the WHOLE grid and probed one by one, so close passages of lenses occur at their true
+    rate (reading R21: the count of rays judged by the close-passage bound is capped at twice its expectation)."""
+    p = CONFIGS[cfg]
+    m, g, xy = make_pair(p)
+    with m:
+        ri, rj = probe_rays(g.n1, g.n2, 250000, p.seed + 50)
+        y_g = m.probe(ri, rj)
+        y_o = oracle.probe(*problem_args(p), xy, ri, rj)
+        cap = max(1, int(2.0 * close_passage_share(g, m.info["tile_w"], xy) * ri.size))
+        r = check_rays(p, g, y_g, y_o, ml.ML_PREC_FP32_TILED, rays_ij=(ri, rj), lenses=xy, tile_w=m.info["tile_w"],
+                       close_passage_cap=cap)
+        r.update(close_passage_cap=cap)
+        report("%s representative sample (250 000 probed rays) fp32_tiled" % p.name, r)
 
 
 def test_c2_full_size_bench_configuration():

@@ -44,7 +44,7 @@ def _worker(rank, world, port, out_dir, precision, ray_mode):
             info = m.info
             m.set_lenses(lens_disk(info["n_star_expected"], info["r_star"], p.seed))
             if ray_mode:
-                m.set_ray_mode(ml.ML_RAYS_RANDOM, 99)
+                m.set_ray_mode(ray_mode, 99)
             info = m.info
             j0, j1 = row_band(info["n2"], rank, world, info["tile_h"])
             m.shoot_region(0, info["n1"], j0, j1)           # the device path of this rank's band
@@ -61,8 +61,10 @@ def _worker(rank, world, port, out_dir, precision, ray_mode):
 
 
 @pytest.mark.parametrize("world", [2, 3])
-@pytest.mark.parametrize("precision,ray_mode", [(ml.ML_PREC_FP32_TILED, 0), (ml.ML_PREC_FP64, 0), (ml.ML_PREC_FP32_TILED, 1)],
-                         ids=["fp32_tiled", "fp64", "fp32_tiled-random_rays"])
+@pytest.mark.parametrize("precision,ray_mode",
+                         [(ml.ML_PREC_FP32_TILED, 0), (ml.ML_PREC_FP64, 0), (ml.ML_PREC_FP32_TILED, ml.ML_RAYS_RANDOM),
+                          (ml.ML_PREC_FP32_TILED, ml.ML_RAYS_UNIFORM)],
+                         ids=["fp32_tiled", "fp64", "fp32_tiled-random_rays", "fp32_tiled-uniform_rays"])
 def test_row_bands_on_the_device_plus_allreduce_equal_the_single_process_map(tmp_path, world, precision, ray_mode):
     mp.spawn(_worker, args=(world, _free_port(), str(tmp_path), precision, ray_mode), nprocs=world, join=True)
     p = CONFIGS[0]
@@ -70,7 +72,7 @@ def test_row_bands_on_the_device_plus_allreduce_equal_the_single_process_map(tmp
         info = m.info
         m.set_lenses(lens_disk(info["n_star_expected"], info["r_star"], p.seed))
         if ray_mode:
-            m.set_ray_mode(ml.ML_RAYS_RANDOM, 99)
+            m.set_ray_mode(ray_mode, 99)
         m.shoot()
         full, st = m.counts(), m.stats
     for r in range(world):

@@ -28,7 +28,7 @@ def _free_port():
         return s.getsockname()[1]
 
 
-def _worker(rank, world, port, out_dir):
+def _worker(rank, world, port, out_dir, ray_mode=None):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
@@ -36,7 +36,8 @@ def _worker(rank, world, port, out_dir):
         xy = lens_disk(g.n_star, g.r_star, 7)
         j0, j1 = row_band(g.n2, rank, world, TILE_H)
         local = np.zeros((ARGS[3], ARGS[3]), dtype=np.uint32)
-        _, st = oracle.shoot_region(*ARGS, xy, region=(0, g.n1, j0, j1), map_out=local)
+        _, st = oracle.shoot_region(*ARGS, xy, region=(0, g.n1, j0, j1), map_out=local,
+                                    ray_seed=None if ray_mode is None else 11, ray_mode=ray_mode)
         counts = torch.from_numpy(local.view(np.int32).copy())
         allreduce_map(counts)
         shot = torch.tensor([st["rays_shot"], st["rays_in_map"]], dtype=torch.int64)
@@ -48,12 +49,15 @@ def _worker(rank, world, port, out_dir):
         dist.destroy_process_group()
 
 
-def test_two_ranks_row_bands_plus_allreduce_equal_the_single_map(tmp_path):
+@pytest.mark.parametrize("ray_mode", [None, "uniform"], ids=["regular", "uniform-rays"])
+def test_two_ranks_row_bands_plus_allreduce_equal_the_single_map(tmp_path, ray_mode):
+    """With uniform rays (reading R20) a row band is a band of ray IDS, not of the image plane: every rank's rays fall
+    all over the rectangle, and the bands still partition the rays."""
     world = 2
-    mp.spawn(_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    mp.spawn(_worker, args=(world, _free_port(), str(tmp_path), ray_mode), nprocs=world, join=True)
     g = oracle.geometry(*ARGS)
     xy = lens_disk(g.n_star, g.r_star, 7)
-    full, st = oracle.shoot(*ARGS, xy)
+    full, st = oracle.shoot(*ARGS, xy, ray_seed=None if ray_mode is None else 11, ray_mode=ray_mode)
     bands = [tuple(np.load(tmp_path / ("band_%d.npy" % r))) for r in range(world)]
     assert bands[0][0] == 0 and bands[0][1] == bands[1][0] and bands[1][1] == g.n2
     assert bands[0][1] % TILE_H == 0

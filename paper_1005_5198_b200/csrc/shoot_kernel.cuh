@@ -150,8 +150,11 @@ __device__ __forceinline__ void ray_uniforms(unsigned long long ray_id, unsigned
 }
 
 // ML_RAYS_UNIFORM (see shoot_kernel_upipe below): bucket size and the ray a list entry stands for
-constexpr int kUniBW = 128, kUniBH = 64; // bucket: grid cells along axis 1 / axis 2 (the FP32 error of a close passage grows
-                                         // with the distance of ray and lens from the local origin: DESIGN.md R15)
+// bucket: grid cells along axis 1 / axis 2.  Small, because the FP32 error of a close passage grows with the distance of ray
+// and lens from the local origin (R15); 128 x 63 = 8064 cells, because a full shoot puts one ray per cell on
+// average and CTAs take 1024 (fp64: 2048) list entries: 8064 + 1.4 sigma = 8192, so 92 % of the buckets need exactly 8 CTAs
+// (at 128 x 64 half of them would need a ninth for a handful of rays).
+constexpr int kUniBW = 128, kUniBH = 63;
 constexpr int kUniWarps = 4;             // shoot_kernel_upipe: 128 threads x 8 rays = 1024 list entries per CTA, 4 CTAs per SM
 
 __host__ __device__ __forceinline__ unsigned long long uniform_ray_id(const ShootParams &p, unsigned long long handle)

@@ -29,7 +29,7 @@ def test_c1_uniform_rays_all_four_criteria(precision):
         m.set_lenses(xy)
         m.set_ray_mode(ml.ML_RAYS_UNIFORM, seed)
         info = m.info
-        assert info["ray_mode"] == ml.ML_RAYS_UNIFORM and info["ray_seed"] == seed and (info["tile_w"], info["tile_h"]) == (128, 64)
+        assert info["ray_mode"] == ml.ML_RAYS_UNIFORM and info["ray_seed"] == seed and (info["tile_w"], info["tile_h"]) == (128, 63)
         m.shoot()
         gmap, gst = m.counts(), m.stats
         omap, ost = oracle.shoot(*problem_args(p), xy, ray_seed=seed, ray_mode="uniform")

@@ -40,7 +40,8 @@ FP32_LANES_PER_SM = 128
 # DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the dominant kernel, from the
 # committed `ncu --set full` capture of this very command; None where no capture exists.
 NCU_DRAM_BYTES_PER_LAUNCH = {
-    ("C2", "fp32_tiled"): (4341504 + 0, "profiles/r01_ncu_full_c2_v2.txt"),
+    ("C2", "fp32_tiled"): (4384512 + 0, "profiles/r02_ncu_full_c2.txt"),
+    ("C2", "fp32_compensated"): (4423168 + 0, "profiles/r02_ncu_full_c2_compensated.txt"),
 }
 NCU_MAPSTATS_DRAM_BYTES = (134337536 + 5088768, "profiles/r01_ncu_full_mapstats.txt")
 

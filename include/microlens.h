@@ -72,8 +72,8 @@ enum {
  *     x = ((i + u1 - n1/2) delta, (j + u2 - n2/2) delta),
  * (u1, u2) = two 53-bit uniforms from Philox-4x32-10 with counter (ray id lo, hi, 0, 0), ray id = j n1 + i,
  * and key = seed (reading R17): the same number of rays, the same mean density, regions and
- * sharding unchanged; the rays share no coordinate differences, so the generic kernel runs
- * (one reciprocal per interaction). */
+ * sharding unchanged; the rays share no coordinate differences, so a kernel with per-ray offsets runs
+ * (shoot_kernel_rpipe in the FP32 modes: 57-60 % of FP32 peak against 74-76 % on the regular grid). */
 enum {
     ML_RAYS_REGULAR = 0,
     ML_RAYS_RANDOM = 1,

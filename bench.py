@@ -42,8 +42,9 @@ FP32_LANES_PER_SM = 128
 NCU_DRAM_BYTES_PER_LAUNCH = {
     ("C2", "fp32_tiled"): (4384512 + 0, "profiles/r02_ncu_full_c2.txt"),
     ("C2", "fp32_compensated"): (4423168 + 0, "profiles/r02_ncu_full_c2_compensated.txt"),
+    ("C2", "fp64"): (4385792 + 0, "profiles/r02_ncu_full_c2_fp64.txt"),
 }
-NCU_MAPSTATS_DRAM_BYTES = (134337536 + 5088768, "profiles/r01_ncu_full_mapstats.txt")
+NCU_MAPSTATS_DRAM_BYTES = (134431232 + 3515904, "profiles/r02_ncu_full_mapstats.txt")
 
 
 def problem_args(p):

@@ -251,7 +251,7 @@ int uniform_run(ml_ctx *c, ShootParams p, long long n_handles, bool capture, uin
         long long rows = (long long)(budget / ((double)nbx * cap * 8.0));
         rows = std::max<long long>(1, std::min(rows, nby - row0));
         if ((double)rows * (double)nbx > 2.0e9) rows = std::max<long long>(1, (long long)(2.0e9 / (double)nbx));
-        const size_t n_b = (size_t)rows * (size_t)nbx, need = ((n_b + 3) & ~(size_t)3) * cap; // (lists interleaved in fours)
+        const size_t n_b = (size_t)rows * (size_t)nbx, need = n_b * cap;
         if (need > c->uni_list_entries) {
             if (c->uni_list) cudaFree(c->uni_list);
             c->uni_list = nullptr;

@@ -59,7 +59,7 @@ struct ShootParams {
     long long n1;             // rays per row of the whole grid (ray id = j*n1 + i, RANDOM instantiations)
     unsigned long long ray_seed; // key of the ray generator (RANDOM instantiations)
     // ---- ML_RAYS_UNIFORM (shoot_kernel_upipe): rays sorted into buckets of kUniBW x kUniBH grid cells
-    const unsigned long long *ray_list; // ray handles of the buckets of this launch, bucket_cap each (uniform_list_index, uniform_ray_id)
+    const unsigned long long *ray_list; // [buckets of this launch][bucket_cap] ray handles (see uniform_ray_id)
     const unsigned int *bucket_fill;    // [buckets of this launch] rays scattered into each bucket (may exceed bucket_cap)
     unsigned int bucket_cap;
     long long bucket_nx, bucket_row0;   // buckets per row of the bucket grid; bucket row of block x = 0
@@ -157,21 +157,6 @@ __device__ __forceinline__ void ray_uniforms(unsigned long long ray_id, unsigned
 constexpr int kUniBW = 128, kUniBH = 63;
 constexpr int kUniWarps = 4;             // shoot_kernel_upipe: 128 threads x 8 rays = 1024 list entries per CTA, 4 CTAs per SM
 
-// Where entry s of bucket b's list lives.  The lists of four consecutive buckets are interleaved sector by sector (4 entries =
-// 32 bytes): while the scatter appends, the open tail of a list is one sector, and four tails share a 128-byte line -- the
-// 1.04e6 tails of C2 are then 33 MB of lines, not 133 MB, and stay in the 126 MB L2 until they are full.
-__host__ __device__ __forceinline__ size_t uniform_list_index(long long b, unsigned int cap, unsigned long long s)
-{
-    return ((size_t)(b >> 2) * cap + (size_t)(s & ~3ull)) * 4 + ((size_t)(b & 3) << 2) + (size_t)(s & 3ull);
-}
-struct HandleList { // a CTA's slice of a bucket list: entries first, first + 1, ...
-    const unsigned long long *list = nullptr;
-    long long b = 0;
-    unsigned int cap = 0;
-    unsigned long long first = 0;
-    __device__ __forceinline__ unsigned long long operator[](int slot) const { return list[uniform_list_index(b, cap, first + (unsigned long long)slot)]; }
-};
-
 __host__ __device__ __forceinline__ unsigned long long uniform_ray_id(const ShootParams &p, unsigned long long handle)
 {
     if (p.probe_ids) return (unsigned long long)p.probe_ids[handle];
@@ -196,7 +181,7 @@ template <int RX, int RY, bool CAPTURE, int WARPS = kWarps, bool RANDOM = false,
 __device__ __forceinline__ void finish_tile(const ShootParams &p, long long ti, long long tj, long long t, int lane,
                                             int warp, const double (&Sx)[RY][RX], const double (&Sy)[RY][RX],
                                             unsigned int *cta_count, const double2 *uv = nullptr, int n_valid = 0,
-                                            const HandleList handles = HandleList())
+                                            const unsigned long long *handles = nullptr)
 {
     constexpr int TW = 32 * RX;
     constexpr int TH = WARPS * RY;
@@ -433,7 +418,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
     long long t = 0, ti = 0, tj = 0;
     int lb, le; // this CTA's lens range: [0, n_lens) except in split capture launches
     int n_valid = 0;
-    HandleList handles;
+    const unsigned long long *handles = nullptr;
     double cx, cy, ccx = 0.0, ccy = 0.0;
     if (UNIFORM) {
         const long long b = (long long)blockIdx.x;
@@ -441,7 +426,7 @@ __global__ void __launch_bounds__(kThreads, 2) shoot_kernel(const ShootParams p)
         const long long first = (long long)blockIdx.y * SLOTS;
         if (first >= (long long)filled) return; // (whole CTA: before any barrier)
         n_valid = (int)min((long long)SLOTS, (long long)filled - first);
-        handles.list = p.ray_list; handles.b = b; handles.cap = p.bucket_cap; handles.first = (unsigned long long)first;
+        handles = p.ray_list + (size_t)b * p.bucket_cap + first;
         lens_range<false>(p, lb, le);
         ccx = (double)((b % p.bucket_nx) * kUniBW) + 0.5 * kUniBW;
         ccy = (double)((p.bucket_row0 + b / p.bucket_nx) * kUniBH) + 0.5 * kUniBH;
@@ -1140,6 +1125,9 @@ constexpr int kScatterRun = 256 * 16;
 __global__ void __launch_bounds__(256) uniform_scatter_kernel(const ScatterParams q)
 {
     const unsigned long long n1 = (unsigned long long)q.sp.n1, n2 = (unsigned long long)q.sp.n2d;
+    // list tails are written 8 bytes at a time: ask the L2 to keep them until their sectors are full
+    unsigned long long keep;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(keep));
     for (long long run = (long long)blockIdx.x * kScatterRun; run < q.n_handles; run += (long long)gridDim.x * kScatterRun) {
         long long h = run + threadIdx.x;
         const long long end = min(run + (long long)kScatterRun, q.n_handles);
@@ -1155,7 +1143,10 @@ __global__ void __launch_bounds__(256) uniform_scatter_kernel(const ScatterParam
             if (by >= q.sp.bucket_row0 && by < q.bucket_row1) {
                 const long long b = (by - q.sp.bucket_row0) * q.sp.bucket_nx + bx;
                 const unsigned int slot = atomicAdd(&q.fill[b], 1u);
-                if (slot < q.sp.bucket_cap) q.list[uniform_list_index(b, q.sp.bucket_cap, slot)] = (unsigned long long)h;
+                if (slot < q.sp.bucket_cap)
+                    asm volatile("st.global.L2::cache_hint.u64 [%0], %1, %2;" ::"l"(q.list + (size_t)b * q.sp.bucket_cap + slot),
+                                 "l"((unsigned long long)h), "l"(keep)
+                                 : "memory");
             }
             ii += 256;
             while (ii >= q.sp.list_w && !q.sp.probe_ids) { ii -= q.sp.list_w; ++jj; }
@@ -1195,8 +1186,7 @@ __global__ void __launch_bounds__(kUniWarps * 32, MINB) shoot_kernel_upipe(const
     const long long first = (long long)blockIdx.y * SLOTS;
     if (first >= (long long)filled) return; // (whole CTA: before any barrier)
     const int n_valid = (int)min((long long)SLOTS, (long long)filled - first);
-    HandleList handles;
-    handles.list = p.ray_list; handles.b = b; handles.cap = p.bucket_cap; handles.first = (unsigned long long)first;
+    const unsigned long long *handles = p.ray_list + (size_t)b * p.bucket_cap + first;
     int lb, le;
     lens_range<false>(p, lb, le);
     if (threadIdx.x < 3) cta_count[threadIdx.x] = 0;

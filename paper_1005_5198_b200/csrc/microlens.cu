@@ -229,6 +229,11 @@ ShootParams base_params(const ml_ctx *c)
     return p;
 }
 
+#ifndef ML_UNIFORM_LIST_BYTES
+#define ML_UNIFORM_LIST_BYTES 0
+#endif
+constexpr long long kUniformListBytes = ML_UNIFORM_LIST_BYTES; // 0: sized from the device memory (below)
+
 // ML_RAYS_UNIFORM: shoot (or capture) the rays behind handles 0 .. n_handles - 1 (p.list_w / p.probe_ids say which).
 // The image plane is cut into buckets of kUniBW x kUniBH grid cells; as many bucket rows as the list memory holds are
 // done per pass: zero the fill counts, scatter the handles (every pass draws every ray again and keeps those of its
@@ -247,7 +252,8 @@ int uniform_run(ml_ctx *c, ShootParams p, long long n_handles, bool capture, uin
         // than what is already held plus what is free less 8 GiB
         size_t free_b = 0, total_b = 0;
         if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) return ML_ERR_CUDA;
-        const double budget = std::min(0.45 * (double)total_b, (double)c->uni_list_entries * 8.0 + (double)free_b - 8.0 * 1073741824.0);
+        double budget = std::min(0.45 * (double)total_b, (double)c->uni_list_entries * 8.0 + (double)free_b - 8.0 * 1073741824.0);
+        if (kUniformListBytes > 0) budget = (double)kUniformListBytes; // (test builds: many passes on a small problem)
         long long rows = (long long)(budget / ((double)nbx * cap * 8.0));
         rows = std::max<long long>(1, std::min(rows, nby - row0));
         if ((double)rows * (double)nbx > 2.0e9) rows = std::max<long long>(1, (long long)(2.0e9 / (double)nbx));

@@ -162,17 +162,23 @@ template <bool CAPTURE> cudaError_t launch(int precision, int ray_mode, dim3 g, 
 
 // uniformly random rays over the whole rectangle (reading R20): bucketed ray lists, one CTA per
 // kUniSlots entries; shoot_kernel_upipe in the FP32 modes, the generic kernel in fp64
+// source-order knobs of shoot_kernel_upipe (same arithmetic, another ptxas schedule), from a sweep of all 32 values on the
+// B200: 29 = accumulations as sx, sx, sy, sy; both lenses' differences before the first r^2; ray pair B's reciprocals
+// first; both 1/r^2 pairs of a row before the first accumulation (C2 step 1397 -> 1382 ms, C4 55.8 -> 56.6 % of FP32 peak)
+#ifndef ML_UPIPE_TUNE
+#define ML_UPIPE_TUNE 29
+#endif
 template <int KF, bool CAPTURE, bool MASS, bool NEWTON> cudaError_t launch_upipe(dim3 g, const ShootParams &p, cudaStream_t s)
 {
     constexpr size_t smem = upipe_smem_bytes(MASS);
     static bool opted_in = false;
     if (!opted_in) {
-        const cudaError_t e = cudaFuncSetAttribute(shoot_kernel_upipe<KF, 4, CAPTURE, MASS, NEWTON>,
+        const cudaError_t e = cudaFuncSetAttribute(shoot_kernel_upipe<KF, 4, CAPTURE, MASS, NEWTON, ML_UPIPE_TUNE>,
                                                    cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         opted_in = true;
     }
-    shoot_kernel_upipe<KF, 4, CAPTURE, MASS, NEWTON><<<g, kUniWarps * 32, smem, s>>>(p);
+    shoot_kernel_upipe<KF, 4, CAPTURE, MASS, NEWTON, ML_UPIPE_TUNE><<<g, kUniWarps * 32, smem, s>>>(p);
     return cudaGetLastError();
 }
 

@@ -1161,7 +1161,11 @@ template <int RY> struct UPipeRegs {   // one row of a thread (two packed ray pa
     float2 R[2];               // shared pairs: 1/(r2[0] r2[1]) per ray pair
 };
 
-template <int KF, int MINB, bool CAPTURE, bool MASS = false, bool NEWTON = false>
+// TUNE: source-order knobs as in the kernels above (same operations, operands and rounding; another ptxas schedule).
+// bit 0: the accumulations of a ray pair as sx, sx, sy, sy instead of sx, sy, sx, sy; bit 1: ray pair B before A in
+// stage 2; bit 2: stage 1 forms the differences of both lenses before the first r^2; bit 3: ray pair B before A in stage 1's
+// reciprocals; bit 4: in stage 2 both 1/r^2 pairs of a row before the first accumulation.
+template <int KF, int MINB, bool CAPTURE, bool MASS = false, bool NEWTON = false, int TUNE = 0>
 __global__ void __launch_bounds__(kUniWarps * 32, MINB) shoot_kernel_upipe(const ShootParams p)
 {
     constexpr int RX = 4, RY = kRandRY, WARPS = kUniWarps;
@@ -1267,17 +1271,21 @@ __global__ void __launch_bounds__(kUniWarps * 32, MINB) shoot_kernel_upipe(const
     // stage 1 of (row r, lens pair l0 l1): differences, r^2, reciprocals (own: of each r^2; shared: of the products)
     auto stage1 = [&](auto own, int r, const float4 l0, const float4 l1, const float m0, const float m1, UPipeRegs<RY> &s) {
         s.m[0] = m0; s.m[1] = m1;
-#pragma unroll
-        for (int L = 0; L < 2; ++L) {
+        auto diffs = [&](int L) {
             const float4 l = L ? l1 : l0;
             const float2 nlx = make_float2(l.x, l.y), nly = make_float2(l.z, l.w);
             s.dx[L][0] = __fadd2_rn(oxA[r], nlx); s.dx[L][1] = __fadd2_rn(oxB[r], nlx);
             s.dy[L][0] = __fadd2_rn(oyA[r], nly); s.dy[L][1] = __fadd2_rn(oyB[r], nly);
+        };
+        auto squares = [&](int L) {
 #pragma unroll
             for (int X = 0; X < 2; ++X) s.r2[L][X] = __ffma2_rn(s.dy[L][X], s.dy[L][X], __ffma2_rn(s.dx[L][X], s.dx[L][X], eps2));
-        }
+        };
+        if (TUNE & 4) { diffs(0); diffs(1); squares(0); squares(1); }
+        else { diffs(0); squares(0); diffs(1); squares(1); }
 #pragma unroll
-        for (int X = 0; X < 2; ++X) {
+        for (int XX = 0; XX < 2; ++XX) {
+            const int X = (TUNE & 8) ? 1 - XX : XX;
             if (decltype(own)::value) {
 #pragma unroll
                 for (int L = 0; L < 2; ++L) {
@@ -1294,9 +1302,8 @@ __global__ void __launch_bounds__(kUniWarps * 32, MINB) shoot_kernel_upipe(const
     };
     // stage 2: 1/r^2 of both lenses and the accumulations, lens 0 before lens 1 (index order)
     auto stage2 = [&](auto own, int r, const UPipeRegs<RY> &s) {
-#pragma unroll
-        for (int X = 0; X < 2; ++X) {
-            float2 i0, i1;
+        float2 i0s[2], i1s[2];
+        auto inv = [&](int X, float2 &i0, float2 &i1) {
             if (decltype(own)::value) {
                 i0 = s.r2[0][X]; i1 = s.r2[1][X];
             } else {
@@ -1306,11 +1313,26 @@ __global__ void __launch_bounds__(kUniWarps * 32, MINB) shoot_kernel_upipe(const
                 i1 = __fmul2_rn(R, s.r2[0][X]);
             }
             if (MASS) { i0 = __fmul2_rn(i0, make_float2(s.m[0], s.m[0])); i1 = __fmul2_rn(i1, make_float2(s.m[1], s.m[1])); }
+        };
+        if (TUNE & 16) { inv(0, i0s[0], i1s[0]); inv(1, i0s[1], i1s[1]); }
+#pragma unroll
+        for (int XX = 0; XX < 2; ++XX) {
+            const int X = (TUNE & 2) ? 1 - XX : XX;
+            float2 i0, i1;
+            if (TUNE & 16) { i0 = i0s[X]; i1 = i1s[X]; }
+            else inv(X, i0, i1);
             float2 &sx = X ? sxB[r] : sxA[r], &sy = X ? syB[r] : syA[r];
-            sx = __ffma2_rn(s.dx[0][X], i0, sx);
-            sy = __ffma2_rn(s.dy[0][X], i0, sy);
-            sx = __ffma2_rn(s.dx[1][X], i1, sx);
-            sy = __ffma2_rn(s.dy[1][X], i1, sy);
+            if (TUNE & 1) {
+                sx = __ffma2_rn(s.dx[0][X], i0, sx);
+                sx = __ffma2_rn(s.dx[1][X], i1, sx);
+                sy = __ffma2_rn(s.dy[0][X], i0, sy);
+                sy = __ffma2_rn(s.dy[1][X], i1, sy);
+            } else {
+                sx = __ffma2_rn(s.dx[0][X], i0, sx);
+                sy = __ffma2_rn(s.dy[0][X], i0, sy);
+                sx = __ffma2_rn(s.dx[1][X], i1, sx);
+                sy = __ffma2_rn(s.dy[1][X], i1, sy);
+            }
         }
     };
 

@@ -70,7 +70,10 @@ struct ShootParams {
 
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
-constexpr int kChunk = 512; // lenses per shared-memory stage
+#ifndef ML_CHUNK
+#define ML_CHUNK 512
+#endif
+constexpr int kChunk = ML_CHUNK; // lenses per shared-memory stage
 
 template <typename Real> struct Vec2;
 template <> struct Vec2<float> { using type = float2; };

@@ -83,7 +83,8 @@ enum {
                             so the counts carry the Poisson noise the paper describes (ML_RAYS_RANDOM's one ray per cell is a
                             stratified sample with less).  (i, j) only numbers the rays: a region of ml_shoot_region /
                             ml_capture_region selects ray ids, not a patch of the image plane.  The library sorts the rays
-                            into buckets of 128 x 63 grid cells on the device (8 bytes of scratch per ray, kept by the context, up to
+                            into buckets of 128 x 63 grid cells on the device (8 bytes of scratch per ray, kept by the context until
+                            ml_destroy or until another ray mode is selected, up to
                             45 % of the device memory; more rays are done in several passes) and shoots each bucket in
                             coordinates local to it; ml_info.tile_w / tile_h report the bucket.  The lens loop is not split
                             over CTAs in this mode. */

@@ -731,6 +731,16 @@ int ml_set_precision(ml_ctx *c, int mode)
 int ml_set_ray_mode(ml_ctx *c, int mode, uint64_t seed)
 {
     if (!c || (mode != ML_RAYS_REGULAR && mode != ML_RAYS_RANDOM && mode != ML_RAYS_UNIFORM)) return ML_ERR_INVALID_ARG;
+    if (mode != ML_RAYS_UNIFORM && c->uni_list) { // leaving the uniform mode: give its bucket lists (8.5 B per ray) back
+        DeviceGuard g(c->device);
+        if (g.ok) {
+            cudaStreamSynchronize(c->stream);
+            cudaFree(c->uni_list);
+            if (c->uni_fill) cudaFree(c->uni_fill);
+            c->uni_list = nullptr; c->uni_fill = nullptr;
+            c->uni_list_entries = 0; c->uni_fill_entries = 0;
+        }
+    }
     c->ray_mode = mode;
     c->ray_seed = mode == ML_RAYS_REGULAR ? 0 : seed;
     return ML_OK;

@@ -38,7 +38,11 @@
  * on C1, Phi bookkeeping of eq.(6)/(9); for the *_m variants: unit masses reproduce the
  * unit-mass path bit for bit, two coincident unit lenses = one lens of mass 2, the Einstein
  * radius of a mass-m lens is sqrt(m), Gauss theorem for a ring of unequal masses, numpy
- * brute force.  No function here is "parity unpinned".
+ * brute force; for the random-ray modes (tests/test_oracle_random_rays.py, tests/test_oracle_uniform_rays.py): the
+ * published Philox known-answer vectors, a second Python restatement of the draws and positions, cell containment
+ * (mode 1) / rectangle coverage and uniformity (mode 2), index of dispersion < 0.5 (mode 1) and 1 (mode 2) on a no-star
+ * map with eq.(12) in the mean, point-lens A(u), region partition by ray id, brute-force maps.
+ * No function here is "parity unpinned".
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/oracle.py).
  * -ffp-contract=off keeps every multiply and add separately rounded, so the

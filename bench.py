@@ -330,6 +330,42 @@ def per_config_entry(ml, torch, name, steps, full_warmup, args, local, flush):
     return out
 
 
+# extra_rows of the default line: the widened rows of DESIGN.md section 11 on C2, one device-timed full step each (after
+# two warm-up shoots of 1/32 of the rows and one full step; the device is warm from the regions before), so that the
+# driver's own run observes them too.  Their full bench lines are `bench.py --masses` etc.
+EXTRA_ROWS = (("C2 unequal masses", {"masses": True}), ("C2 random rays, one per cell (R17)", {"random_rays": True}),
+              ("C2 uniform rays over the whole rectangle (R20), position sort included", {"uniform_rays": True}),
+              ("C2 fp32_compensated", {"precision": "fp32_compensated"}), ("C2 fp64", {"precision": "fp64"}))
+
+
+def extra_row(ml, torch, label, overrides, args, local, flush):
+    a = argparse.Namespace(**vars(args))
+    for k, v in overrides.items():
+        setattr(a, k, v)
+    p = pick("C2")
+    rig = ShootRig(ml, torch, p, a, local, flush=flush)
+    band = max(int(rig.info["tile_h"]), rig.n2 // 32)
+    for k in range(2):
+        rig.step(rows=(k * band, (k + 1) * band))
+    rig.step()                                   # one full step: also sizes the uniform mode's bucket lists
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    rig.flush_l2()
+    e0.record(rig.stream)
+    rig.m.shoot_region(0, rig.n1, 0, rig.n2)
+    e1.record(rig.stream)
+    torch.cuda.synchronize(rig.dev)
+    st = rig.m.stats
+    assert int(st["rays_shot"]) == rig.n1 * rig.n2
+    ms = e0.elapsed_time(e1)
+    peak, _ = fp32_peak_tflops(rig.info)
+    inter = float(rig.n1) * rig.n2 * rig.n_lens
+    out = {"row": label, "steps": 1, "ms_per_step": ms, "kernel_ms": st["kernel_ms"], "gpu_launches": int(st["kernel_launches"]),
+           "value": inter / (ms * 1e-3), "unit": UNIT, "frac": N_FLOP * inter / (st["kernel_ms"] * 1e-3) / 1e12 / peak,
+           "precision": a.precision}
+    rig.close()
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -438,6 +474,17 @@ def run_ours(args):
                        "clocks": clocks, "note": "the line's own timed region"}]
         for name, steps, full_warmup in PER_CONFIG_PLAN:
             per_config.append(per_config_entry(ml, torch, name, steps, full_warmup, args, local, flush))
+    extra = None
+    if per_config is not None:
+        extra = [extra_row(ml, torch, label, ov, args, local, flush) for label, ov in EXTRA_ROWS]
+        del flush
+        torch.cuda.empty_cache()
+        ms_args = argparse.Namespace(**vars(args))
+        ms_args.steps, ms_args.warmup, ms_args.no_cpu_baseline = 10, 3, True
+        ml_line = mapstats_line(ms_args)
+        extra.append({"row": "map comparison of two 4096^2 maps (ml_map_compare)", "steps": 10, "ms_per_step": ml_line["ms_per_step"],
+                      "value": ml_line["value"], "unit": ml_line["unit"], "frac": ml_line["roofline"]["frac"], "bound": "hbm",
+                      "pass_kernel_ms": ml_line["roofline"]["pass_kernel_ms"], "call_ms_without_flush": ml_line["call_ms_without_flush"]})
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         cpu = oracle_rate(p, args.cpu_seconds)
@@ -454,6 +501,7 @@ def run_ours(args):
             "gpu_launches": launches_all}
     if per_config is not None:
         line["per_config"] = per_config
+        line["extra_rows"] = extra
     print(json.dumps(line))
     return 0
 
@@ -477,12 +525,17 @@ def spawn_ranks(args):
 
 # ------------------------------------------------------------------ the map-comparison row
 def run_mapstats(args):
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    print(json.dumps(mapstats_line(args)))
+    return 0
+
+
+def mapstats_line(args):
     """--row mapstats: pixels/s of ml_map_compare (RMS in magnitudes + two-sample K-S) on two
     seeded synthetic 4096^2 count maps (the map size of C4) resident in HBM; HBM roofline."""
     import torch
     import paper_1005_5198_b200 as ml
-    if int(os.environ.get("RANK", "0")) != 0:
-        return 0
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
@@ -575,8 +628,7 @@ def run_mapstats(args):
                     "d2h_bytes_per_step": 112},
             "gpu_launches": 7 * args.steps,   # pass, reduce, three scan kernels, K-S, finalize (+ one memset) per call
             "call_ms_without_flush": call_ms}
-    print(json.dumps(line))
-    return 0
+    return line
 
 
 def main():

@@ -53,7 +53,9 @@ enum {
     ML_ERR_INVALID_ARG = -1, /* bad argument (see each call)                        */
     ML_ERR_CUDA = -2,        /* a CUDA runtime call failed / no device              */
     ML_ERR_OOM = -3,         /* host or device allocation failed                    */
-    ML_ERR_STATE = -4        /* call sequence error (e.g. shoot before set_lenses)  */
+    ML_ERR_STATE = -4,       /* call sequence error (e.g. shoot before set_lenses)  */
+    ML_ERR_LIMIT = -5        /* the input needs more than the fixed built-in scratch of a call that never
+                                allocates (ml_delta_m_histogram_static)                */
 };
 
 /* Arithmetic of the deflection sum (eq.8 leaves the summation order open;
@@ -253,6 +255,48 @@ int ml_map_compare(const uint32_t *a, double n_rays_a, const uint32_t *b, double
  * [lo, hi) and empty pixels are not counted.  ML_ERR_INVALID_ARG unless lo < hi, 1 <= n_bins <= 2^20. */
 int ml_delta_m_histogram(const uint32_t *counts, double n_rays, int64_t n, double lo, double hi,
                          int32_t n_bins, int where, int32_t device, void *cuda_stream, uint64_t *hist_out);
+
+/* ml_delta_m_histogram for callers that must not allocate device memory.
+ *
+ * Who that is: a program that has handed (nearly) all of the GPU's memory to its own pool before it calls in here -- a
+ * torch process whose caching allocator already holds the HBM, an inference server that reserved its arena at start-up --
+ * so that a late cudaMalloc inside this library fails although the program itself still has room; and a program that
+ * renders maps in a loop next to other GPU work and cannot accept that cudaMalloc / cudaFree stall every stream of the
+ * device while they run.  ml_delta_m_histogram keeps a growing per-device cache (count histogram, partial sums, a
+ * staging copy of the output) that it cudaMalloc's on first use and when a map is brighter than anything seen before.
+ * This variant computes the same histogram with the same kernels but takes its scratch from a fixed array that is part
+ * of the library image (a file-scope __device__ array in csrc/mapstats.cu); it calls no cudaMalloc, cudaFree,
+ * cudaMallocHost, cudaEventCreate or any other allocating routine, on any call.
+ *
+ *   counts    DEVICE, n uint32 counts (e.g. the pointer of ml_get_map_device, or a torch tensor)       -- input, read only
+ *   hist_out  DEVICE, n_bins uint64, 8-byte aligned, owned by the caller -- output; the call overwrites all n_bins
+ *             entries (whatever was there before is discarded) with the histogram ml_delta_m_histogram defines
+ *   n_rays, n, lo, hi, n_bins, device, cuda_stream: as for ml_delta_m_histogram.  There is no `where`: host pointers are
+ *             not accepted, because staging them would need a device buffer.
+ *
+ * The limit.  The built-in scratch is ML_STATIC_SCRATCH_BYTES (1 MiB + 16 KiB): a count histogram of
+ * ML_STATIC_MAX_COUNT = 2^18 bins, 256 per-CTA partial sums and one totals record.  Every GPU on which this process
+ * uses the library holds that array from the moment the library's code is loaded on it until the process exits,
+ * whether or not this function is ever called.  Therefore every count must be < ML_STATIC_MAX_COUNT (262144; the
+ * BASELINE configs peak below 1e5).  A brighter pixel is detected on the device and the call returns ML_ERR_LIMIT
+ * ("more than the built-in scratch holds"); hist_out is then unspecified.  Use ml_delta_m_histogram for such maps.
+ * ML_ERR_INVALID_ARG for NULL / misaligned pointers and for the argument errors of ml_delta_m_histogram;
+ * ML_ERR_CUDA if a runtime call fails.
+ *
+ * Set-up.  The first call on each device looks up the device address of the built-in array (cudaGetSymbolAddress with
+ * that device current) and raises the pass kernel's shared-memory limit; later calls on that device reuse both.
+ * Make that first call early, outside any stream capture: it is the only one that talks to the driver about more than
+ * launches and memsets.
+ *
+ * Sharing.  All calls on a device use the one array, and it keeps what the previous call left in it; each call clears
+ * the part that has to start at zero on `cuda_stream` before its kernels run.  Two calls whose GPU work overlaps would
+ * corrupt each other's histograms.  Inside one process that cannot happen -- a call holds the library's lock until it
+ * has synchronised `cuda_stream` -- but nothing orders this call against GPU work the caller has queued on OTHER
+ * streams: do not let such work write `counts` or touch `hist_out` while the call runs. */
+#define ML_STATIC_MAX_COUNT (1u << 18)
+#define ML_STATIC_SCRATCH_BYTES ((1u << 20) + (1u << 14))
+int ml_delta_m_histogram_static(const uint32_t *counts, double n_rays, int64_t n, double lo, double hi,
+                                int32_t n_bins, int32_t device, void *cuda_stream, uint64_t *hist_out);
 
 /* Static description of a return code. */
 const char *ml_strerror(int code);

@@ -8,6 +8,7 @@ from .binding import (  # noqa: F401
     EXPORTS,
     ML_ERR_CUDA,
     ML_ERR_INVALID_ARG,
+    ML_ERR_LIMIT,
     ML_ERR_OOM,
     ML_ERR_STATE,
     ML_MEM_DEVICE,
@@ -19,6 +20,7 @@ from .binding import (  # noqa: F401
     ML_RAYS_RANDOM,
     ML_RAYS_REGULAR,
     ML_RAYS_UNIFORM,
+    ML_STATIC_MAX_COUNT,
     MicrolensError,
     library_path,
     load,
@@ -26,6 +28,7 @@ from .binding import (  # noqa: F401
     ml_capture_region,
     ml_create,
     ml_delta_m_histogram,
+    ml_delta_m_histogram_static,
     ml_destroy,
     ml_get_info,
     ml_get_map,

@@ -19,6 +19,8 @@ ML_ERR_INVALID_ARG = -1
 ML_ERR_CUDA = -2
 ML_ERR_OOM = -3
 ML_ERR_STATE = -4
+ML_ERR_LIMIT = -5
+ML_STATIC_MAX_COUNT = 1 << 18
 
 ML_PREC_FP32_TILED = 0
 ML_PREC_FP32_COMPENSATED = 1
@@ -29,6 +31,7 @@ EXPORTS = (
     "ml_shoot_region", "ml_get_map", "ml_get_map_device", "ml_use_device_map", "ml_attach_stream",
     "ml_get_stats", "ml_capture_region", "ml_probe", "ml_strerror", "ml_version",
     "ml_map_compare", "ml_delta_m_histogram", "ml_set_lens_masses", "ml_set_ray_mode",
+    "ml_delta_m_histogram_static",
 )
 
 ML_RAYS_REGULAR = 0
@@ -120,6 +123,7 @@ def load():
     u32p = C.POINTER(C.c_uint32)
     lib.ml_map_compare.argtypes = [vp, dbl, vp, dbl, i64, C.c_int, i32, vp, C.POINTER(MlMapCompareResult)]
     lib.ml_delta_m_histogram.argtypes = [vp, dbl, i64, dbl, dbl, i32, C.c_int, i32, vp, C.POINTER(C.c_uint64)]
+    lib.ml_delta_m_histogram_static.argtypes = [vp, dbl, i64, dbl, dbl, i32, i32, vp, vp]
     del u32p
     lib.ml_strerror.argtypes = [C.c_int]
     lib.ml_strerror.restype = C.c_char_p
@@ -282,3 +286,17 @@ def ml_delta_m_histogram(counts, n_rays, lo, hi, n_bins, n=None, device=0, cuda_
                                        C.c_void_p(int(cuda_stream) if cuda_stream else None),
                                        out.ctypes.data_as(C.POINTER(C.c_uint64))), "ml_delta_m_histogram")
     return out
+
+
+def ml_delta_m_histogram_static(counts_ptr, n_rays, n, lo, hi, n_bins, hist_out_ptr, device=0, cuda_stream=None) -> None:
+    """ml_delta_m_histogram without a single device allocation inside the library, for programs whose own pool
+    (torch's caching allocator, a server's arena) already owns the GPU memory or that cannot take the device-wide
+    stall of cudaMalloc / cudaFree.  counts_ptr: int DEVICE pointer to n uint32 counts; hist_out_ptr: int DEVICE
+    pointer to n_bins uint64 the caller allocated (e.g. tensor.data_ptr() of a torch int64 tensor) -- overwritten.
+    Scratch is a fixed 1 MiB array inside the library: every count must be < ML_STATIC_MAX_COUNT (2^18), else
+    MicrolensError with code ML_ERR_LIMIT.  The first call on a device does a one-time symbol look-up; make it
+    before any stream capture.  See include/microlens.h."""
+    _check(load().ml_delta_m_histogram_static(C.c_void_p(int(counts_ptr)), float(n_rays), int(n), float(lo), float(hi),
+                                              int(n_bins), int(device),
+                                              C.c_void_p(int(cuda_stream) if cuda_stream else None),
+                                              C.c_void_p(int(hist_out_ptr))), "ml_delta_m_histogram_static")

@@ -653,3 +653,90 @@ int ml_delta_m_histogram(const uint32_t *counts, double n_rays, int64_t n, doubl
 }
 
 } // extern "C"
+
+// ---------------------------------------------------------------------------------------- no-allocation variant
+// ml_delta_m_histogram_static (include/microlens.h): the same pass / reduce / Delta-m kernels as ml_delta_m_histogram,
+// but their scratch is this fixed array inside the library image instead of the cudaMalloc'ed per-device cache above.
+// For callers whose process cannot (its own pool owns the memory) or must not (cudaMalloc / cudaFree stall the whole
+// device) allocate.  Each device that loads this module holds ML_STATIC_SCRATCH_BYTES for it until the process exits.
+namespace {
+
+constexpr unsigned int kStaticBins = ML_STATIC_MAX_COUNT; // bins of the count histogram: counts must stay below this
+constexpr int kStaticMaxBlocks = 256;                     // per-CTA partial sums (the pass runs one CTA per SM, at most this many)
+
+struct StaticLayout {
+    unsigned int hist[kStaticBins];       // must be zero when the pass starts: cleared on the stream by every call
+    Partial partials[kStaticMaxBlocks];   // [0, grid) fully rewritten by the pass
+    Totals totals;                        // fully rewritten by reduce_partials_kernel
+};
+static_assert(sizeof(StaticLayout) <= ML_STATIC_SCRATCH_BYTES, "the documented size of the built-in scratch is too small");
+
+// NOTE for host code: `g_static_scratch` names the host-side shadow of the symbol, not device memory.  Passing it to a
+// kernel would fault (or quietly use host memory on systems where the GPU can reach it).  Host code below only ever
+// uses the address cudaGetSymbolAddress returns for the current device.
+static __device__ __align__(256) unsigned char g_static_scratch[ML_STATIC_SCRATCH_BYTES];
+
+struct StaticDevice {
+    bool ready = false;
+    int sm_count = 0;
+    StaticLayout *scratch = nullptr; // device address of g_static_scratch on this device
+};
+StaticDevice g_static[kMaxDevices];
+
+// Once per device, with that device current (the caller holds a DeviceScope and g_lock).  Allocates nothing.
+int static_setup(StaticDevice &sd, int device)
+{
+    if (sd.ready) return ML_OK;
+    void *ptr = nullptr;
+    if (cudaGetSymbolAddress(&ptr, g_static_scratch) != cudaSuccess || !ptr) { cudaGetLastError(); return ML_ERR_CUDA; }
+    if (cudaDeviceGetAttribute(&sd.sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) { cudaGetLastError(); return ML_ERR_CUDA; }
+    // per-device attribute; the allocating path sets the same value in Scratch::init, so the order of first use does not matter
+    if (cudaFuncSetAttribute(pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPassSmem) != cudaSuccess) {
+        cudaGetLastError();
+        return ML_ERR_CUDA;
+    }
+    sd.scratch = static_cast<StaticLayout *>(ptr);
+    sd.ready = true;
+    return ML_OK;
+}
+
+} // namespace
+
+extern "C" int ml_delta_m_histogram_static(const uint32_t *counts, double n_rays, int64_t n, double lo, double hi, int32_t n_bins,
+                                           int32_t device, void *cuda_stream, uint64_t *hist_out)
+{
+    if (!counts || !hist_out || (reinterpret_cast<uintptr_t>(counts) & 3) || (reinterpret_cast<uintptr_t>(hist_out) & 7) || n < 1 ||
+        n > 0x7fffffffLL || bad_rays(n_rays) || !(lo < hi) || !isfinite(lo) || !isfinite(hi) || n_bins < 1 || n_bins > (1 << 20))
+        return ML_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    DeviceScope g(device);
+    if (!g.ok) return ML_ERR_CUDA;
+    std::lock_guard<std::mutex> hold(g_lock); // one call at a time per process: every call works in the same array
+    StaticDevice &sd = g_static[device];
+    int rc = static_setup(sd, device);
+    if (rc != ML_OK) return rc;
+    StaticLayout *sc = sd.scratch;
+    int grid = grid_for(n, sd.sm_count);
+    if (grid > kStaticMaxBlocks) grid = kStaticMaxBlocks; // a device with more SMs than partial-sum slots: grid-stride loop covers the rest
+    // the array still holds the previous call's histogram: clear it (stream-ordered), and the caller's output bins
+    if (cudaMemsetAsync(sc->hist, 0, sizeof(sc->hist), s) != cudaSuccess ||
+        cudaMemsetAsync(hist_out, 0, (size_t)n_bins * sizeof(uint64_t), s) != cudaSuccess) {
+        cudaGetLastError();
+        return ML_ERR_CUDA;
+    }
+    pass_kernel<false><<<grid, kPassThreads, kPassSmem, s>>>(counts, nullptr, n, n_rays, n_rays, sc->hist, nullptr, kStaticBins, sc->partials,
+                                                             nullptr);
+    reduce_partials_kernel<<<1, 32, 0, s>>>(sc->partials, grid, kStaticBins, &sc->totals);
+    const int want = (int)(kStaticBins / kThreads);
+    delta_m_hist_kernel<<<want < sd.sm_count * 8 ? want : sd.sm_count * 8, kThreads, 0, s>>>(
+        sc->hist, &sc->totals, n_rays, lo, hi, n_bins, reinterpret_cast<unsigned long long *>(hist_out));
+    if (cudaGetLastError() != cudaSuccess) return ML_ERR_CUDA;
+    // 4 bytes back into a stack variable (pageable: the runtime stages the copy itself, nothing is allocated here)
+    unsigned int overflow = 0;
+    if (cudaMemcpyAsync(&overflow, &sc->totals.overflow, sizeof(overflow), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        cudaStreamSynchronize(s) != cudaSuccess) {
+        cudaGetLastError();
+        return ML_ERR_CUDA;
+    }
+    return overflow ? ML_ERR_LIMIT : ML_OK; // a count >= ML_STATIC_MAX_COUNT was not histogrammed
+}

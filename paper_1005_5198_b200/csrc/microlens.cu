@@ -919,6 +919,7 @@ const char *ml_strerror(int code)
     case ML_ERR_CUDA: return "CUDA runtime error or no CUDA device";
     case ML_ERR_OOM: return "out of memory";
     case ML_ERR_STATE: return "call sequence error (lenses not set)";
+    case ML_ERR_LIMIT: return "the input needs more than the built-in scratch of a no-allocation entry point holds";
     default: return "unknown error code";
     }
 }

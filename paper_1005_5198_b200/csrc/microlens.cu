@@ -8,6 +8,7 @@
 #include "shoot_kernel.cuh"
 
 #include <algorithm>
+#include <atomic>
 #include <chrono>
 #include <cmath>
 #include <cstring>
@@ -122,18 +123,29 @@ template <bool CAPTURE, bool MASS> cudaError_t launch_m(int precision, dim3 g, c
 #ifndef ML_RPIPE_TUNE
 #define ML_RPIPE_TUNE 10
 #endif
+// More than 48 KB of dynamic shared memory needs cudaFuncAttributeMaxDynamicSharedMemorySize, and that attribute belongs to
+// the (function, device) pair: a process that shoots from contexts on several GPUs has to opt in on each of them.  `done`
+// (one per kernel instantiation) has bit d set once device d is done; the launch runs with the context's device current.
+template <typename Kernel> cudaError_t opt_in_shared_memory(Kernel kernel, size_t smem, std::atomic<unsigned long long> &done)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const bool tracked = dev >= 0 && dev < 64;
+    if (tracked && ((done.load(std::memory_order_acquire) >> dev) & 1ull)) return cudaSuccess;
+    e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); // idempotent: a race repeats it harmlessly
+    if (e == cudaSuccess && tracked) done.fetch_or(1ull << dev, std::memory_order_release);
+    return e;
+}
+
 // random ray positions (reading R17): the packed random-ray kernel in the FP32 modes, the generic
 // kernel with per-ray offsets in fp64
 template <int KF, bool CAPTURE, bool MASS, bool NEWTON> cudaError_t launch_rpipe(dim3 g, const ShootParams &p, cudaStream_t s)
 {
     constexpr size_t smem = rpipe_smem_bytes(MASS);
-    static bool opted_in = false; // more than 48 KB of dynamic shared memory needs the opt-in once per function
-    if (!opted_in) {
-        const cudaError_t e = cudaFuncSetAttribute(shoot_kernel_rpipe<KF, 2, CAPTURE, MASS, NEWTON, ML_RPIPE_OWN, ML_RPIPE_TUNE>,
-                                                   cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        opted_in = true;
-    }
+    static std::atomic<unsigned long long> opted_in{0ull}; // per device, see opt_in_shared_memory
+    const cudaError_t e = opt_in_shared_memory(shoot_kernel_rpipe<KF, 2, CAPTURE, MASS, NEWTON, ML_RPIPE_OWN, ML_RPIPE_TUNE>, smem, opted_in);
+    if (e != cudaSuccess) return e;
     shoot_kernel_rpipe<KF, 2, CAPTURE, MASS, NEWTON, ML_RPIPE_OWN, ML_RPIPE_TUNE><<<g, kRandWarps * 32, smem, s>>>(p);
     return cudaGetLastError();
 }
@@ -171,13 +183,9 @@ template <bool CAPTURE> cudaError_t launch(int precision, int ray_mode, dim3 g, 
 template <int KF, bool CAPTURE, bool MASS, bool NEWTON> cudaError_t launch_upipe(dim3 g, const ShootParams &p, cudaStream_t s)
 {
     constexpr size_t smem = upipe_smem_bytes(MASS);
-    static bool opted_in = false;
-    if (!opted_in) {
-        const cudaError_t e = cudaFuncSetAttribute(shoot_kernel_upipe<KF, 4, CAPTURE, MASS, NEWTON, ML_UPIPE_TUNE>,
-                                                   cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        opted_in = true;
-    }
+    static std::atomic<unsigned long long> opted_in{0ull}; // per device, see opt_in_shared_memory
+    const cudaError_t e = opt_in_shared_memory(shoot_kernel_upipe<KF, 4, CAPTURE, MASS, NEWTON, ML_UPIPE_TUNE>, smem, opted_in);
+    if (e != cudaSuccess) return e;
     shoot_kernel_upipe<KF, 4, CAPTURE, MASS, NEWTON, ML_UPIPE_TUNE><<<g, kUniWarps * 32, smem, s>>>(p);
     return cudaGetLastError();
 }
@@ -411,6 +419,11 @@ int shoot_split(ml_ctx *c, ShootParams p, const Mode &m, long long ti0, long lon
 constexpr long long kMaxGridX = ML_MAX_GRID_X, kMaxGridY = ML_MAX_GRID_Y;
 static_assert(kMaxGridX >= 1 && kMaxGridX <= 0x7fffffffLL && kMaxGridY >= 1 && kMaxGridY <= 65535LL, "grid limits");
 
+int shoot_region_run(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1, int accumulate);
+
+// The device counters are running totals; `seen` (their value after the last shoot) becomes the next run's `base`.  A run
+// that fails after some of its kernels were enqueued has already moved the totals, so on every error exit they are read
+// again (best effort): otherwise the next run's rays_shot / rays_in_map / interactions would include the failed run's rays.
 int shoot_region_impl(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1, int accumulate)
 {
     if (!c) return ML_ERR_INVALID_ARG;
@@ -418,6 +431,20 @@ int shoot_region_impl(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1,
     if (i0 < 0 || j0 < 0 || i1 > c->n1 || j1 > c->n2 || i0 > i1 || j0 > j1) return ML_ERR_INVALID_ARG;
     DeviceGuard g(c->device);
     if (!g.ok) return ML_ERR_CUDA;
+    const int rc = shoot_region_run(c, i0, i1, j0, j1, accumulate);
+    if (rc != ML_OK) {
+        cudaGetLastError();
+        if (cudaMemcpyAsync(c->h_counters, c->counters, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream) == cudaSuccess &&
+            cudaStreamSynchronize(c->stream) == cudaSuccess)
+            std::memcpy(c->seen, c->h_counters, sizeof(c->seen));
+        else
+            cudaGetLastError();
+    }
+    return rc;
+}
+
+int shoot_region_run(ml_ctx *c, int64_t i0, int64_t i1, int64_t j0, int64_t j1, int accumulate)
+{
     const auto t0 = std::chrono::steady_clock::now();
     if (!accumulate) {
         // one memset: the counters are running totals and are never zeroed (the run's statistics are differences)

@@ -43,6 +43,10 @@ def build_library(force: bool = False, verbose: bool = False, defines=(), out: s
 
     `defines` (e.g. ["ML_MAX_GRID_Y=50"]) and `out` make a separate TEST build of the same sources (the
     launch-split test uses one); such a build is loaded by pointing MICROLENS_B200_LIBRARY at it (binding.load)."""
+    if defines and (out is None or os.path.abspath(out) == os.path.abspath(LIB_PATH)):
+        # such a library would be newer than its sources, so is_stale() would keep it: every later load (bench, tests)
+        # would silently run the test build
+        raise ValueError("build_library: `defines` make a test build and need an `out` other than the shipped %s" % LIB_PATH)
     target = out or LIB_PATH
     if not out and not defines and not force and not is_stale():
         return LIB_PATH

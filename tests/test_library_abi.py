@@ -93,3 +93,15 @@ def test_product_never_imports_the_oracle():
             if f.endswith((".py", ".cu", ".cuh", ".h", ".cpp")):
                 text = open(os.path.join(dirpath, f)).read()
                 assert "oracle" not in text.lower(), (dirpath, f)
+
+
+def test_test_builds_cannot_overwrite_the_shipped_library(tmp_path):
+    """build_library(defines=...) makes a crippled TEST build (tiny grid limits, tiny list memory).  Written over the
+    shipped .so it would be newer than its sources and every later load would silently use it: refused."""
+    from paper_1005_5198_b200 import build as mlbuild
+    before = os.path.getmtime(mlbuild.LIB_PATH)
+    with pytest.raises(ValueError):
+        mlbuild.build_library(defines=["ML_MAX_GRID_X=7"])
+    with pytest.raises(ValueError):
+        mlbuild.build_library(defines=["ML_MAX_GRID_X=7"], out=mlbuild.LIB_PATH)
+    assert os.path.getmtime(mlbuild.LIB_PATH) == before

@@ -10,7 +10,7 @@ import paper_1005_5198_b200 as ml
 from oracle import oracle
 from workloads import CONFIGS, lens_disk, lens_masses
 
-from parity_common import (PREC_NAME, check_maps, check_rays, close_passage_share, problem_args, report, run_subregions,
+from parity_common import (PREC_NAME, check_maps, check_rays, problem_args, report, run_subregions,
                            subregion_tiles)
 
 pytestmark = pytest.mark.gpu
@@ -37,9 +37,8 @@ def test_c1_uniform_rays_all_four_criteria(precision):
         y_g = m.capture_region(0, g.n1, 0, g.n2)
         y_o = oracle.capture_region(*problem_args(p), xy, (0, g.n1, 0, g.n2), ray_seed=seed, ray_mode="uniform")
         ii, jj = np.meshgrid(np.arange(g.n1, dtype=np.int64), np.arange(g.n2, dtype=np.int64))
-        cap = max(1, int(2.0 * close_passage_share(g, info["tile_w"], xy) * ii.size))
         r.update(check_rays(p, g, y_g, y_o, precision, rays_ij=(ii, jj), lenses=xy, ray_seed=seed, tile_w=info["tile_w"],
-                            ray_mode="uniform", close_passage_cap=cap), close_passage_cap=cap)
+                            ray_mode="uniform", representative=True))
         # the list order inside a bucket follows the atomics, the arithmetic of a ray does not: same bits every time
         m.shoot()
         assert np.array_equal(m.counts(), gmap)

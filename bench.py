@@ -43,12 +43,26 @@ NCU_DRAM_BYTES_PER_LAUNCH = {
     ("C2", "fp32_tiled"): (4384512 + 0, "profiles/r02_ncu_full_c2.txt"),
     ("C2", "fp32_compensated"): (4423168 + 0, "profiles/r02_ncu_full_c2_compensated.txt"),
     ("C2", "fp64"): (4385792 + 0, "profiles/r02_ncu_full_c2_fp64.txt"),
+    # widened rows (key: workload, precision, row): the shoot kernel of that row
+    ("C2", "fp32_tiled", "random_rays"): (5490000, "profiles/r02_ncu_full_c2_random.txt"),
+    ("C2", "fp32_tiled", "uniform_rays"): (68970000000 + 750000000, "profiles/r02_ncu_full_c2_uniform.txt (shoot_kernel_upipe; "
+                                           "the scatter kernel moves another 283 GB, r02_ncu_full_c2_uniform_scatter.txt)"),
 }
 NCU_MAPSTATS_DRAM_BYTES = (134431232 + 3515904, "profiles/r02_ncu_full_mapstats.txt")
 
 
 def problem_args(p):
     return (p.sigma, p.stellar_fraction, p.gamma, p.n_pix, p.n_rays, p.L)
+
+
+def sig(x, digits=6):
+    """A float rounded to `digits` significant digits: the per_config / extra_rows blocks must fit the ~5 KB tail of
+    stdout that the driver's record keeps."""
+    return float("%.*g" % (digits, x))
+
+
+def brief_clocks(clocks):
+    return {"sm_mhz": clocks.get("sm_mhz"), "reasons": clocks.get("reasons")} if clocks else None
 
 
 def pick(name):
@@ -143,6 +157,8 @@ def run_reference(args):
     if rank != 0:
         return 0
     p = pick(args.workload)
+    from oracle import oracle
+    g = oracle.geometry(*problem_args(p))
     per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
     if args.ref_seconds_per_step is not None:
         per_step = args.ref_seconds_per_step
@@ -158,7 +174,9 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
             "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": config_dict(p, None, args),
+            "data": "synthetic", "config": config_dict(p, {"n_lenses": g.n_star, "n1": g.n1, "n2": g.n2}, args),
+            "precision": "fp64", "config_note": "config is the CUDA arm's, key for key (its l2 / parallelism entries describe that arm; "
+                                                  "this arm runs the oracle on the host cores)",
             "cpu_baseline": base,
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -180,10 +198,10 @@ def config_dict(p, info, args):
                          "PAPER.md:131, :167; reading R20): bucket sort on the device + shoot_kernel_upipe, both inside the step")
     if getattr(args, "n_lenses", 0) > 0:
         c["n_lenses_override"] = "lens count set to %d in the same disk (large-N* row, not a BASELINE config)" % args.n_lenses
+    # the geometry keys are the same in both arms (ours: ml_get_info; --impl reference: the oracle's own geometry), so
+    # that the two `config` objects are identical; what differs between the arms (precision, tile) is top-level
     if info is not None:
-        c.update(n_lenses=int(info["n_lenses"]), n1=int(info["n1"]), n2=int(info["n2"]),
-                 rays=int(info["n1"]) * int(info["n2"]), tile=[int(info["tile_w"]), int(info["tile_h"])],
-                 precision=args.precision)
+        c.update(n_lenses=int(info["n_lenses"]), n1=int(info["n1"]), n2=int(info["n2"]), rays=int(info["n1"]) * int(info["n2"]))
     return c
 
 
@@ -271,7 +289,9 @@ class ShootRig:
 
 
 def per_config_entry(ml, torch, name, steps, full_warmup, args, local, flush):
-    """One entry of the default line's per_config block (single GPU).  Every timed step is an END-TO-END step (host
+    """One entry of the default line's per_config block (single GPU; keys kept short, see `sig`: unit = the line's unit,
+    e2e_value / e2e_ms = the end-to-end rate and wall time per step with h2d / d2h bytes copied per step; each config is
+    shot 2 x steps times, once end to end and once device-timed).  Every timed step is an END-TO-END step (host
     lenses -> ml_set_lenses -> ml_shoot -> ml_get_map -> host map, L2 flushed before it, outside the clock): `e2e` is
     its wall clock, `kernel_ms` the library's CUDA events around the kernel launch of the same step, `value` the
     device-timed rate of the whole step without the copies (memset + kernel, events on the launching stream)."""
@@ -318,14 +338,12 @@ def per_config_entry(ml, torch, name, steps, full_warmup, args, local, flush):
     inter = float(rays) * n_lens
     h2d, d2h = rig.e2e_bytes()
     k_ms = kernel_ms / (2 * steps)
-    out = {"workload": config_dict(p, rig.info, args)["workload"], "n_lenses": n_lens, "rays": rays, "steps": steps,
-           "kernel_ms": k_ms, "ms_per_step": dev_ms / steps, "value": inter * steps / (dev_ms * 1e-3), "unit": UNIT,
-           "frac": N_FLOP * inter / (k_ms * 1e-3) / 1e12 / peak,
-           "step_frac": N_FLOP * inter * steps / (dev_ms * 1e-3) / 1e12 / peak,
-           "e2e": {"value": inter * steps / wall, "unit": UNIT, "ms_per_step": 1e3 * wall / steps,
-                   "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-           "clocks": clocks,
-           "note": "each config is shot 2 x steps times: once end to end (host buffers, wall clock) and once device-timed"}
+    out = {"workload": p.name, "n_lenses": n_lens, "rays": rays, "steps": steps,
+           "kernel_ms": sig(k_ms), "ms_per_step": sig(dev_ms / steps), "value": sig(inter * steps / (dev_ms * 1e-3)),
+           "frac": sig(N_FLOP * inter / (k_ms * 1e-3) / 1e12 / peak, 4),
+           "step_frac": sig(N_FLOP * inter * steps / (dev_ms * 1e-3) / 1e12 / peak, 4),
+           "e2e_value": sig(inter * steps / wall), "e2e_ms": sig(1e3 * wall / steps),
+           "h2d": h2d, "d2h": d2h, "clocks": brief_clocks(clocks)}
     rig.close()
     return out
 
@@ -333,8 +351,8 @@ def per_config_entry(ml, torch, name, steps, full_warmup, args, local, flush):
 # extra_rows of the default line: the widened rows of DESIGN.md section 11 on C2, one device-timed full step each (after
 # two warm-up shoots of 1/32 of the rows and one full step; the device is warm from the regions before), so that the
 # driver's own run observes them too.  Their full bench lines are `bench.py --masses` etc.
-EXTRA_ROWS = (("C2 unequal masses", {"masses": True}), ("C2 random rays, one per cell (R17)", {"random_rays": True}),
-              ("C2 uniform rays over the whole rectangle (R20), position sort included", {"uniform_rays": True}),
+EXTRA_ROWS = (("C2 masses", {"masses": True}), ("C2 random rays (R17)", {"random_rays": True}),
+              ("C2 uniform rays (R20), sort included", {"uniform_rays": True}),
               ("C2 fp32_compensated", {"precision": "fp32_compensated"}), ("C2 fp64", {"precision": "fp64"}))
 
 
@@ -359,9 +377,8 @@ def extra_row(ml, torch, label, overrides, args, local, flush):
     ms = e0.elapsed_time(e1)
     peak, _ = fp32_peak_tflops(rig.info)
     inter = float(rig.n1) * rig.n2 * rig.n_lens
-    out = {"row": label, "steps": 1, "ms_per_step": ms, "kernel_ms": st["kernel_ms"], "gpu_launches": int(st["kernel_launches"]),
-           "value": inter / (ms * 1e-3), "unit": UNIT, "frac": N_FLOP * inter / (st["kernel_ms"] * 1e-3) / 1e12 / peak,
-           "precision": a.precision}
+    out = {"row": label, "ms_per_step": sig(ms), "kernel_ms": sig(st["kernel_ms"]), "gpu_launches": int(st["kernel_launches"]),
+           "value": sig(inter / (ms * 1e-3)), "frac": sig(N_FLOP * inter / (st["kernel_ms"] * 1e-3) / 1e12 / peak, 4)}
     rig.close()
     return out
 
@@ -453,25 +470,26 @@ def run_ours(args):
     # ncu DRAM bytes exist only for the exact kernel that was captured: the BASELINE workload, unit masses, regular grid
     plain = world == 1 and not (args.masses or args.random_rays or args.uniform_rays or args.n_lenses > 0)
     traffic, traffic_src = NCU_DRAM_BYTES_PER_LAUNCH.get((p.name, args.precision), (None, None)) if plain else (None, None)
+    if world == 1 and not plain and not args.masses and args.n_lenses <= 0 and not (args.random_rays and args.uniform_rays):
+        row = "random_rays" if args.random_rays else "uniform_rays"
+        traffic, traffic_src = NCU_DRAM_BYTES_PER_LAUNCH.get((p.name, args.precision, row), (None, None))
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved / peak_tflops, "traffic": traffic,
-                "traffic_unit": "bytes of DRAM traffic per launch (ncu --set full; %s); algorithmic HBM bytes per "
-                                "launch = n_pix^2*4 map + 16*N* lenses = %d"
+                "traffic_unit": "DRAM bytes per launch (ncu --set full; %s); algorithmic = n_pix^2*4 + 16 N* = %d"
                                 % (traffic_src or "no capture of this kernel instantiation", p.n_pix * p.n_pix * 4 + 16 * n_lens),
-                "note": "nominal %g flop/interaction (PAPER.md:66); peak = %d SMs x 128 FP32 lanes x 2 x %.0f MHz "
-                        "(MEASURED_PEAKS.json sm_max_mhz); kernel time = CUDA events on the launching stream"
-                        % (N_FLOP, sm_count, max_mhz),
+                "note": "%g flop/interaction (PAPER.md:66); peak = %d SMs x 128 lanes x 2 x %.0f MHz (sm_max_mhz); "
+                        "kernel time = CUDA events on the launching stream" % (N_FLOP, sm_count, max_mhz),
                 "kernel_ms_per_launch": 1e3 * kernel_s_per_launch}
     if clocks and clocks.get("sm_mhz"):
         roofline["frac_at_sampled_clock"] = achieved / (peak_tflops * clocks["sm_mhz"] / max_mhz)
     per_config = None
     if plain and args.workload == "C2" and args.precision == "fp32_tiled" and not args.no_per_config:
-        per_config = [{"workload": config_dict(p, info, args)["workload"], "n_lenses": n_lens, "rays": n1 * n2,
-                       "steps": args.steps, "kernel_ms": 1e3 * kernel_s_per_launch, "ms_per_step": ms / args.steps,
-                       "value": value, "unit": UNIT, "frac": achieved / peak_tflops,
-                       "step_frac": N_FLOP * value / 1e12 / peak_tflops,
-                       "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-                       "clocks": clocks, "note": "the line's own timed region"}]
+        per_config = [{"workload": p.name, "n_lenses": n_lens, "rays": n1 * n2,        # the line's own timed region
+                       "steps": args.steps, "kernel_ms": sig(1e3 * kernel_s_per_launch), "ms_per_step": sig(ms / args.steps),
+                       "value": sig(value), "frac": sig(achieved / peak_tflops, 4),
+                       "step_frac": sig(N_FLOP * value / 1e12 / peak_tflops, 4),
+                       "e2e_value": sig(e2e_value), "e2e_ms": sig(1e3 * float(e2e_t[0]) / e2e_steps),
+                       "h2d": h2d, "d2h": d2h, "clocks": brief_clocks(clocks)}]
         for name, steps, full_warmup in PER_CONFIG_PLAN:
             per_config.append(per_config_entry(ml, torch, name, steps, full_warmup, args, local, flush))
     extra = None
@@ -482,9 +500,9 @@ def run_ours(args):
         ms_args = argparse.Namespace(**vars(args))
         ms_args.steps, ms_args.warmup, ms_args.no_cpu_baseline = 10, 3, True
         ml_line = mapstats_line(ms_args)
-        extra.append({"row": "map comparison of two 4096^2 maps (ml_map_compare)", "steps": 10, "ms_per_step": ml_line["ms_per_step"],
-                      "value": ml_line["value"], "unit": ml_line["unit"], "frac": ml_line["roofline"]["frac"], "bound": "hbm",
-                      "pass_kernel_ms": ml_line["roofline"]["pass_kernel_ms"], "call_ms_without_flush": ml_line["call_ms_without_flush"]})
+        extra.append({"row": "ml_map_compare, two 4096^2 maps", "ms_per_step": sig(ml_line["ms_per_step"]),
+                      "value": sig(ml_line["value"]), "unit": ml_line["unit"], "frac": sig(ml_line["roofline"]["frac"], 4), "bound": "hbm",
+                      "pass_kernel_ms": sig(ml_line["roofline"]["pass_kernel_ms"]), "call_ms_without_flush": sig(ml_line["call_ms_without_flush"])})
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         cpu = oracle_rate(p, args.cpu_seconds)
@@ -493,6 +511,7 @@ def run_ours(args):
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
             "scaling": "strong", "vs_baseline": None, "dtype": "f32" if args.precision != "fp64" else "f64",
             "data": "synthetic", "config": config_dict(p, info, args),
+            "precision": args.precision, "tile": [int(info["tile_w"]), int(info["tile_h"])],
             "rays_per_s": rays_all / (ms * 1e-3), "map_wall_ms": ms / args.steps,
             "nominal_tflops": N_FLOP * value / 1e12, "frac_fp32_peak": N_FLOP * value / 1e12 / (peak_tflops * args.gpus),
             "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,

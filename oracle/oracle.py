@@ -66,7 +66,8 @@ _lib = None
 def _load():
     global _lib
     if _lib is None:
-        lib = C.CDLL(build())
+        # ML_ORACLE_LIBRARY: another build of the same C file (tests/test_oracle_sanitizers.py loads an ASan/UBSan one)
+        lib = C.CDLL(os.environ.get("ML_ORACLE_LIBRARY") or build())
         dp = C.POINTER(C.c_double)
         ip = C.POINTER(C.c_int64)
         pp = C.POINTER(_Problem)

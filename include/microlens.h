@@ -144,7 +144,10 @@ void ml_destroy(ml_ctx *ctx);
 int ml_get_info(const ml_ctx *ctx, ml_info *out);
 
 /* Lens positions (PAPER.md:130 step 1, :138): xy = n interleaved (x, y) HOST fp64
- * pairs in Einstein radii, unit masses.  Copied to the device; the caller keeps xy.
+ * pairs in Einstein radii, unit masses.  Copied before the call returns (into a pinned
+ * staging buffer of the context, and from there to the device on the context's stream,
+ * ordered before the next shoot; the call does not wait for the device and, once its
+ * buffers have grown to the largest field seen, allocates nothing); the caller keeps xy.
  * n >= 0 and need not equal n_star_expected (n = 0: no stars).  A non-finite
  * coordinate gives ML_ERR_INVALID_ARG and leaves the previous lenses in place. */
 int ml_set_lenses(ml_ctx *ctx, const double *xy, int64_t n);
@@ -154,7 +157,8 @@ int ml_set_lenses(ml_ctx *ctx, const double *xy, int64_t n);
  * paper sets all masses equal).  The deflection of lens i is m_i (x - xi_i)/|x - xi_i|^2;
  * the kernels multiply 1/r^2 by m_i (one extra FP32 multiply per ray pair and lens).  For a mean mass
  * <M> the lens count of eq.5 is n_star_expected / <M>.  ML_ERR_INVALID_ARG for a non-finite or
- * non-positive mass; the previous lenses stay in place on any error. */
+ * non-positive mass; the previous lenses stay in place on ML_ERR_INVALID_ARG and ML_ERR_OOM (after
+ * ML_ERR_CUDA no lenses are set). */
 int ml_set_lens_masses(ml_ctx *ctx, const double *xy, const double *mass, int64_t n);
 
 /* Select ML_RAYS_* (see the enum); seed keys the generator of ML_RAYS_RANDOM / ML_RAYS_UNIFORM and is ignored otherwise.

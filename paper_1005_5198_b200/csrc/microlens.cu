@@ -33,6 +33,13 @@ struct ml_ctx {
     double2 *lens;
     double *mass;     // device masses m_i (eq.4), nullptr = unit masses
     int64_t n_lenses; // -1: never set
+    // ml_set_lenses without a device allocation or a synchronisation per call: device buffers and a pinned staging copy
+    // that only grow, and an event that says when the staging copy may be overwritten
+    size_t lens_cap, mass_cap;      // elements the device buffers `lens` / `mass_buf` hold
+    double *mass_buf;               // device masses buffer (kept when a later call sets unit masses); `mass` = it or nullptr
+    unsigned char *h_stage;         // pinned: [n double2 | n double]
+    size_t stage_bytes;
+    cudaEvent_t ev_stage;           // recorded after the copies out of h_stage
     unsigned long long *counters; // device [3]: running totals, never reset (a shoot reports the difference)
     unsigned long long *h_counters; // pinned host copy of the same
     unsigned long long seen[3];     // device totals after the last shoot
@@ -681,7 +688,9 @@ void ml_destroy(ml_ctx *c)
             if (c->own_stream) cudaStreamSynchronize(c->own_stream);
             if (c->map_own) cudaFree(c->map_own);
             if (c->lens) cudaFree(c->lens);
-            if (c->mass) cudaFree(c->mass);
+            if (c->mass_buf) cudaFree(c->mass_buf);
+            if (c->h_stage) cudaFreeHost(c->h_stage);
+            if (c->ev_stage) cudaEventDestroy(c->ev_stage);
             if (c->counters) cudaFree(c->counters);
             if (c->h_counters) cudaFreeHost(c->h_counters);
             if (c->h_uni_max) cudaFreeHost(c->h_uni_max);
@@ -722,25 +731,54 @@ int ml_set_lens_masses(ml_ctx *c, const double *xy, const double *mass, int64_t 
             if (!std::isfinite(mass[k]) || !(mass[k] > 0.0)) return ML_ERR_INVALID_ARG;
     DeviceGuard g(c->device);
     if (!g.ok) return ML_ERR_CUDA;
+    // The caller's arrays are copied into the pinned staging buffer before returning (the caller keeps xy / mass, pinned or
+    // not), and from there to the device on the context's stream: the next shoot is ordered after the copy, nothing waits
+    // here.  Every buffer only grows, so a map-per-lens-field loop allocates nothing after its first pass.  The stream is
+    // idle whenever this runs (every shoot / capture ends with a synchronisation), so the lens array is not in use.
+    const size_t cnt = (size_t)std::max<int64_t>(n, 1);
+    const size_t need_stage = cnt * (sizeof(double2) + sizeof(double));
+    if (c->ev_stage && cudaEventSynchronize(c->ev_stage) != cudaSuccess) { cudaGetLastError(); return ML_ERR_CUDA; } // previous copy out of h_stage
+    if (need_stage > c->stage_bytes) {
+        unsigned char *h = nullptr;
+        if (cudaMallocHost(&h, need_stage) != cudaSuccess) { cudaGetLastError(); return ML_ERR_OOM; }
+        if (c->h_stage) cudaFreeHost(c->h_stage);
+        c->h_stage = h;
+        c->stage_bytes = need_stage;
+    }
+    if (!c->ev_stage && cudaEventCreateWithFlags(&c->ev_stage, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return ML_ERR_CUDA; }
+    // grow the device buffers: both allocations first, so that on failure the previous lenses are still in place
     double2 *d = nullptr;
     double *dm = nullptr;
-    if (cudaMalloc(&d, (size_t)std::max<int64_t>(n, 1) * sizeof(double2)) != cudaSuccess ||
-        (mass && cudaMalloc(&dm, (size_t)std::max<int64_t>(n, 1) * sizeof(double)) != cudaSuccess)) {
+    if ((cnt > c->lens_cap && cudaMalloc(&d, cnt * sizeof(double2)) != cudaSuccess) ||
+        (mass && cnt > c->mass_cap && cudaMalloc(&dm, cnt * sizeof(double)) != cudaSuccess)) {
         cudaGetLastError();
         if (d) cudaFree(d);
         return ML_ERR_OOM;
     }
-    if (n > 0 && (cudaMemcpyAsync(d, xy, (size_t)n * sizeof(double2), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
-                  (mass && cudaMemcpyAsync(dm, mass, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, c->stream) != cudaSuccess) ||
-                  cudaStreamSynchronize(c->stream) != cudaSuccess)) {
-        cudaFree(d);
-        if (dm) cudaFree(dm);
-        return ML_ERR_CUDA;
+    if (d) {
+        if (c->lens) cudaFree(c->lens); // (synchronises the device: only when a larger field arrives)
+        c->lens = d;
+        c->lens_cap = cnt;
     }
-    if (c->lens) cudaFree(c->lens);
-    if (c->mass) cudaFree(c->mass);
-    c->lens = d;
-    c->mass = dm;
+    if (dm) {
+        if (c->mass_buf) cudaFree(c->mass_buf);
+        c->mass_buf = dm;
+        c->mass_cap = cnt;
+    }
+    double2 *h_xy = reinterpret_cast<double2 *>(c->h_stage);
+    double *h_m = reinterpret_cast<double *>(c->h_stage + cnt * sizeof(double2));
+    if (n > 0) {
+        std::memcpy(h_xy, xy, (size_t)n * sizeof(double2));
+        if (mass) std::memcpy(h_m, mass, (size_t)n * sizeof(double));
+        if (cudaMemcpyAsync(c->lens, h_xy, (size_t)n * sizeof(double2), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
+            (mass && cudaMemcpyAsync(c->mass_buf, h_m, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, c->stream) != cudaSuccess) ||
+            cudaEventRecord(c->ev_stage, c->stream) != cudaSuccess) {
+            cudaGetLastError();
+            c->n_lenses = -1; // the device array may hold a mixture now: ml_shoot refuses until lenses are set again
+            return ML_ERR_CUDA;
+        }
+    }
+    c->mass = mass ? c->mass_buf : nullptr;
     c->n_lenses = n;
     return ML_OK;
 }
@@ -822,6 +860,11 @@ int ml_use_device_map(ml_ctx *c, void *dptr)
 int ml_attach_stream(ml_ctx *c, void *cuda_stream)
 {
     if (!c) return ML_ERR_INVALID_ARG;
+    if (c->ev_stage && (cudaStream_t)cuda_stream != c->stream) {
+        // lenses set on the previous stream may still be on their way to the device: the new stream waits for that copy
+        DeviceGuard g(c->device);
+        if (!g.ok || cudaStreamWaitEvent((cudaStream_t)cuda_stream, c->ev_stage, 0) != cudaSuccess) { cudaGetLastError(); return ML_ERR_CUDA; }
+    }
     c->stream = (cudaStream_t)cuda_stream;
     return ML_OK;
 }

@@ -226,3 +226,48 @@ def test_caller_owned_torch_map_and_stream():
         torch.cuda.synchronize()
         assert np.array_equal(t.cpu().numpy().astype(np.uint32), ref) and int(t2.sum()) < int(t.sum())
         m.use_device_map(0)
+
+
+def test_set_lenses_is_stream_ordered_and_keeps_nothing_of_the_callers_buffer():
+    """ml_set_lenses returns without waiting for the device and reuses its buffers (a map-per-lens-field loop allocates
+    nothing after the first pass).  It must still have copied the caller's arrays by the time it returns -- also when
+    they are PINNED, where an asynchronous copy would read them later -- and a sequence of larger and smaller fields, with
+    and without masses, on changing streams, must give the maps a fresh context gives for each field."""
+    import torch
+    p = SMALL
+    g = oracle.geometry(*problem_args(p))
+
+    def fresh(xy, mass=None):
+        with ml.MagnificationMap(*problem_args(p)) as f:
+            f.set_lenses(xy, mass)
+            f.shoot()
+            return f.counts().copy()
+
+    fields = [(lens_disk(g.n_star, g.r_star, 3), None),
+              (lens_disk(4 * g.n_star + 3, g.r_star, 4), lens_masses(4 * g.n_star + 3, 4)),   # grows, masses appear
+              (lens_disk(7, g.r_star, 5), None),                                              # shrinks, unit masses again
+              (lens_disk(2 * g.n_star, g.r_star, 6), lens_masses(2 * g.n_star, 6)),           # masses buffer reused
+              (np.zeros((0, 2)), None)]                                                        # no stars
+    want = [fresh(xy, mass) for xy, mass in fields]
+    assert not np.array_equal(want[0], want[1]) and not np.array_equal(want[2], want[3])
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    with ml.MagnificationMap(*problem_args(p)) as m:
+        for k, (xy, mass) in enumerate(fields):
+            t_xy = torch.from_numpy(xy.copy()).pin_memory()
+            t_m = torch.from_numpy(mass.copy()).pin_memory() if mass is not None else None
+            m.set_lenses(t_xy.numpy(), t_m.numpy() if t_m is not None else None)
+            t_xy.fill_(123.0)                      # the caller's (pinned) arrays are the caller's again
+            if t_m is not None:
+                t_m.fill_(50.0)
+            if k % 2 == 1:                         # lenses set on one stream, shot on another
+                m.attach_stream(streams[(k // 2) % 2].cuda_stream)
+            m.shoot()
+            assert m.info["n_lenses"] == xy.shape[0]
+            assert np.array_equal(m.counts(), want[k]), k
+        # a rejected field leaves the last one (no stars) in place
+        bad = fields[0][0].copy()
+        bad[1, 0] = np.inf
+        with pytest.raises(ml.MicrolensError):
+            m.set_lenses(bad)
+        m.shoot()
+        assert np.array_equal(m.counts(), want[-1])

@@ -40,6 +40,10 @@ struct ml_ctx {
     unsigned char *h_stage;         // pinned: [n double2 | n double]
     size_t stage_bytes;
     cudaEvent_t ev_stage;           // recorded after the copies out of h_stage
+    // device scratch of probes / captures / split-lens shoots (tile lists, captured positions, partial sums): kept between
+    // calls while small, so that a probe loop does not pay two device-synchronising allocator calls per probe
+    void *scratch[3];
+    size_t scratch_bytes[3];
     unsigned long long *counters; // device [3]: running totals, never reset (a shoot reports the difference)
     unsigned long long *h_counters; // pinned host copy of the same
     unsigned long long seen[3];     // device totals after the last shoot
@@ -71,6 +75,44 @@ struct DeviceGuard {
         if (ok) cudaSetDevice(prev);
     }
 };
+
+// Device scratch for one call (see ml_ctx::scratch).  Slots up to kKeepScratchBytes stay with the context and only grow;
+// a larger request is allocated for this call alone and freed when the lease ends (a context does not sit on gigabytes
+// because of one large capture).  Every user synchronises the stream before its lease ends, so a kept slot is idle
+// between calls.
+constexpr size_t kKeepScratchBytes = 64ull << 20;
+struct ScratchLease {
+    void *ptr = nullptr;
+    bool own = false; // allocated for this call only
+    ScratchLease() = default;
+    ScratchLease(const ScratchLease &) = delete;
+    ScratchLease &operator=(const ScratchLease &) = delete;
+    ~ScratchLease()
+    {
+        if (own && ptr) cudaFree(ptr);
+    }
+    // false: out of memory (nothing leased)
+    bool take(ml_ctx *c, int slot, size_t bytes)
+    {
+        if (bytes == 0) bytes = 1;
+        if (bytes > kKeepScratchBytes) {
+            own = cudaMalloc(&ptr, bytes) == cudaSuccess;
+            if (!own) { cudaGetLastError(); ptr = nullptr; }
+            return own;
+        }
+        if (bytes > c->scratch_bytes[slot]) {
+            if (c->scratch[slot]) cudaFree(c->scratch[slot]);
+            c->scratch[slot] = nullptr;
+            c->scratch_bytes[slot] = 0;
+            if (cudaMalloc(&c->scratch[slot], bytes) != cudaSuccess) { cudaGetLastError(); c->scratch[slot] = nullptr; return false; }
+            c->scratch_bytes[slot] = bytes;
+        }
+        ptr = c->scratch[slot];
+        return true;
+    }
+    template <typename T> T *as() const { return static_cast<T *>(ptr); }
+};
+enum { kSlotList = 0, kSlotBuf = 1, kSlotPart = 2 };
 
 // Tile shape and kernel instantiations per precision mode.
 struct Mode {
@@ -254,6 +296,17 @@ ShootParams base_params(const ml_ctx *c)
 #define ML_UNIFORM_LIST_BYTES 0
 #endif
 constexpr long long kUniformListBytes = ML_UNIFORM_LIST_BYTES; // 0: sized from the device memory (below)
+#ifndef ML_UNIFORM_FAIL_ALLOCS
+#define ML_UNIFORM_FAIL_ALLOCS 0
+#endif
+// (test builds: the first ML_UNIFORM_FAIL_ALLOCS list allocations of the process report failure, to drive the retry below)
+inline bool uniform_alloc_fails_in_this_test_build()
+{
+    static int left = ML_UNIFORM_FAIL_ALLOCS;
+    if (left <= 0) return false;
+    --left;
+    return true;
+}
 
 // ML_RAYS_UNIFORM: shoot (or capture) the rays behind handles 0 .. n_handles - 1 (p.list_w / p.probe_ids say which).
 // The image plane is cut into buckets of kUniBW x kUniBH grid cells; as many bucket rows as the list memory holds are
@@ -278,12 +331,22 @@ int uniform_run(ml_ctx *c, ShootParams p, long long n_handles, bool capture, uin
         long long rows = (long long)(budget / ((double)nbx * cap * 8.0));
         rows = std::max<long long>(1, std::min(rows, nby - row0));
         if ((double)rows * (double)nbx > 2.0e9) rows = std::max<long long>(1, (long long)(2.0e9 / (double)nbx));
-        const size_t n_b = (size_t)rows * (size_t)nbx, need = n_b * cap;
+        size_t n_b = (size_t)rows * (size_t)nbx, need = n_b * cap;
         if (need > c->uni_list_entries) {
             if (c->uni_list) cudaFree(c->uni_list);
             c->uni_list = nullptr;
             c->uni_list_entries = 0;
-            if (cudaMalloc(&c->uni_list, need * sizeof(unsigned long long)) != cudaSuccess) { cudaGetLastError(); return ML_ERR_OOM; }
+            // cudaMemGetInfo is a snapshot: another context or a caching allocator on the same device may have taken the
+            // memory since.  A stripe of half as many bucket rows needs half the list: retry down to one row.
+            for (;;) {
+                if (!uniform_alloc_fails_in_this_test_build() && cudaMalloc(&c->uni_list, need * sizeof(unsigned long long)) == cudaSuccess) break;
+                cudaGetLastError();
+                c->uni_list = nullptr;
+                if (rows <= 1) return ML_ERR_OOM;
+                rows = (rows + 1) / 2;
+                n_b = (size_t)rows * (size_t)nbx;
+                need = n_b * cap;
+            }
             c->uni_list_entries = need;
         }
         if (n_b + 1 > c->uni_fill_entries) {
@@ -371,7 +434,7 @@ int plan_lens_split(const ml_ctx *c, long long nb, long long max_splits, int *sp
 
 // ml_shoot_region over a handful of tiles and very many lenses: the capture instantiation (which bins nothing) runs
 // once per (tile, lens range) and leaves fp64 partial sums; combine_kernel<.., CAPTURE = false> adds them in range
-// order and bins the rays with the region masks.  Synchronises (the partial sums are freed before returning).
+// order and bins the rays with the region masks.  Synchronises (the scratch is idle again when it returns).
 int shoot_split(ml_ctx *c, ShootParams p, const Mode &m, long long ti0, long long tj0, long long tiles_x, long long tiles_y,
                 int n_splits, int split_len, float *ms)
 {
@@ -387,28 +450,26 @@ int shoot_split(ml_ctx *c, ShootParams p, const Mode &m, long long ti0, long lon
     } catch (const std::bad_alloc &) {
         return ML_ERR_OOM;
     }
-    long long *d_list = nullptr;
-    double2 *d_part = nullptr;
+    ScratchLease list, part;
     int rc = ML_OK;
-    if (cudaMalloc(&d_list, tiles.size() * sizeof(long long)) != cudaSuccess ||
-        cudaMalloc(&d_part, (size_t)n_splits * n_tiles * m.tw * m.th * sizeof(double2)) != cudaSuccess) {
-        cudaGetLastError();
+    if (!list.take(c, kSlotList, tiles.size() * sizeof(long long)) ||
+        !part.take(c, kSlotPart, (size_t)n_splits * n_tiles * m.tw * m.th * sizeof(double2)))
         rc = ML_ERR_OOM;
-    }
     if (rc == ML_OK) {
+        long long *d_list = list.as<long long>();
         p.tile_list = d_list;
         p.split_len = split_len;
-        p.partial = d_part;
+        p.partial = part.as<double2>();
         if (cudaMemcpyAsync(d_list, tiles.data(), tiles.size() * sizeof(long long), cudaMemcpyHostToDevice, c->stream) != cudaSuccess ||
             cudaEventRecord(c->ev0, c->stream) != cudaSuccess ||
             launch<true>(c->precision, c->ray_mode, dim3((unsigned int)n_tiles, (unsigned int)n_splits, 1), p, c->stream) != cudaSuccess ||
             launch_combine<false>(c->precision, c->ray_mode, (unsigned int)n_tiles, p, n_splits, c->stream) != cudaSuccess ||
             cudaEventRecord(c->ev1, c->stream) != cudaSuccess || cudaStreamSynchronize(c->stream) != cudaSuccess ||
-            cudaEventElapsedTime(ms, c->ev0, c->ev1) != cudaSuccess)
+            cudaEventElapsedTime(ms, c->ev0, c->ev1) != cudaSuccess) {
             rc = ML_ERR_CUDA;
+            cudaStreamSynchronize(c->stream); // the leases end below: nothing may still be running in them
+        }
     }
-    if (d_list) cudaFree(d_list);
-    if (d_part) cudaFree(d_part);
     if (rc == ML_OK) c->stats.capture_ctas = (uint64_t)n_tiles * (uint64_t)n_splits;
     return rc;
 }
@@ -522,8 +583,7 @@ int capture_tiles(ml_ctx *c, const std::vector<long long> &tiles /* pairs */, Si
     const long long batch = std::max<long long>(1, std::min<long long>(n_tiles, (256ll << 20) / (long long)(per_tile * sizeof(double2))));
     int split_len = 0;
     const int n_splits = plan_lens_split(c, batch, (1024ll << 20) / (long long)(batch * per_tile * sizeof(double2)), &split_len);
-    long long *d_list = nullptr;
-    double2 *d_buf = nullptr, *d_part = nullptr;
+    ScratchLease list, buf, part;
     std::vector<double2> h_buf;
     try {
         h_buf.resize((size_t)batch * per_tile);
@@ -531,12 +591,11 @@ int capture_tiles(ml_ctx *c, const std::vector<long long> &tiles /* pairs */, Si
         return ML_ERR_OOM;
     }
     int rc = ML_OK;
-    if (cudaMalloc(&d_list, tiles.size() * sizeof(long long)) != cudaSuccess ||
-        cudaMalloc(&d_buf, (size_t)batch * per_tile * sizeof(double2)) != cudaSuccess ||
-        (n_splits > 1 && cudaMalloc(&d_part, (size_t)n_splits * batch * per_tile * sizeof(double2)) != cudaSuccess)) {
-        cudaGetLastError();
-        rc = ML_ERR_OOM;
-    }
+    if (!list.take(c, kSlotList, tiles.size() * sizeof(long long)) || !buf.take(c, kSlotBuf, (size_t)batch * per_tile * sizeof(double2)) ||
+        (n_splits > 1 && !part.take(c, kSlotPart, (size_t)n_splits * batch * per_tile * sizeof(double2))))
+        return ML_ERR_OOM;
+    long long *d_list = list.as<long long>();
+    double2 *d_buf = buf.as<double2>(), *d_part = part.as<double2>();
     if (rc == ML_OK && cudaMemcpyAsync(d_list, tiles.data(), tiles.size() * sizeof(long long), cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
         rc = ML_ERR_CUDA;
     for (long long first = 0; rc == ML_OK && first < n_tiles; first += batch) {
@@ -562,23 +621,18 @@ int capture_tiles(ml_ctx *c, const std::vector<long long> &tiles /* pairs */, Si
         c->stats.capture_ctas = n_splits > 1 ? (uint64_t)nb * (uint64_t)n_splits : 0;
         sink(first, nb, h_buf.data());
     }
-    cudaFree(d_list);
-    cudaFree(d_buf);
-    if (d_part) cudaFree(d_part);
+    if (rc != ML_OK) cudaStreamSynchronize(c->stream); // the leases end here: nothing may still be running in them
     return rc;
 }
 
 // ML_RAYS_UNIFORM: positions of the rays behind handles 0 .. n - 1 (region-relative indices, or entries of `ids`).
 int capture_uniform(ml_ctx *c, ShootParams p, long long n, const std::vector<long long> *ids, double *y_out)
 {
-    double2 *d_buf = nullptr;
-    long long *d_ids = nullptr;
+    ScratchLease buf, idl;
+    if (!buf.take(c, kSlotBuf, (size_t)n * sizeof(double2)) || (ids && !idl.take(c, kSlotList, (size_t)n * sizeof(long long)))) return ML_ERR_OOM;
+    double2 *d_buf = buf.as<double2>();
+    long long *d_ids = ids ? idl.as<long long>() : nullptr;
     int rc = ML_OK;
-    if (cudaMalloc(&d_buf, (size_t)n * sizeof(double2)) != cudaSuccess ||
-        (ids && cudaMalloc(&d_ids, (size_t)n * sizeof(long long)) != cudaSuccess)) {
-        cudaGetLastError();
-        rc = ML_ERR_OOM;
-    }
     if (rc == ML_OK && ids &&
         cudaMemcpyAsync(d_ids, ids->data(), (size_t)n * sizeof(long long), cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
         rc = ML_ERR_CUDA;
@@ -591,8 +645,7 @@ int capture_uniform(ml_ctx *c, ShootParams p, long long n, const std::vector<lon
     if (rc == ML_OK && (cudaMemcpyAsync(y_out, d_buf, (size_t)n * sizeof(double2), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess ||
                         cudaStreamSynchronize(c->stream) != cudaSuccess))
         rc = ML_ERR_CUDA;
-    if (d_buf) cudaFree(d_buf);
-    if (d_ids) cudaFree(d_ids);
+    if (rc != ML_OK) cudaStreamSynchronize(c->stream); // the leases end here: nothing may still be running in them
     return rc;
 }
 
@@ -689,6 +742,8 @@ void ml_destroy(ml_ctx *c)
             if (c->map_own) cudaFree(c->map_own);
             if (c->lens) cudaFree(c->lens);
             if (c->mass_buf) cudaFree(c->mass_buf);
+            for (void *q : c->scratch)
+                if (q) cudaFree(q);
             if (c->h_stage) cudaFreeHost(c->h_stage);
             if (c->ev_stage) cudaEventDestroy(c->ev_stage);
             if (c->counters) cudaFree(c->counters);

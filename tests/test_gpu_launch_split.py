@@ -67,7 +67,10 @@ def _run_child(tmp, lib=None):
 
 
 def test_a_build_with_tiny_grid_limits_reproduces_the_map_bit_for_bit(tmp_path):
-    lib = mlbuild.build_library(defines=["ML_MAX_GRID_X=7", "ML_MAX_GRID_Y=50", "ML_UNIFORM_LIST_BYTES=4194304"],
+    # ML_UNIFORM_FAIL_ALLOCS=2: the first two allocations of the uniform mode's bucket lists "fail", so the run also goes
+    # through the retry with half (then a quarter) of the bucket rows per stripe instead of returning ML_ERR_OOM
+    lib = mlbuild.build_library(defines=["ML_MAX_GRID_X=7", "ML_MAX_GRID_Y=50", "ML_UNIFORM_LIST_BYTES=4194304",
+                                         "ML_UNIFORM_FAIL_ALLOCS=2"],
                                 out=str(tmp_path / "libmicrolens_split.so"))
     normal = _run_child(str(tmp_path / "normal"))
     split = _run_child(str(tmp_path / "split"), lib)

@@ -407,6 +407,10 @@ def run_ours(args):
     p = pick(args.workload)
     rig = ShootRig(ml, torch, p, args, local, rank, world)
     info, n1, n2, n_lens, stream = rig.info, rig.n1, rig.n2, rig.n_lens, rig.stream
+    if world > 1:   # one line per rank on stderr, so that a scaling record shows the N ranks, their devices and bands
+        print("bench.py: rank %d/%d on cuda:%d (%s), communicator size %d, ray rows [%d, %d) of %d"
+              % (rank, world, local, torch.cuda.get_device_name(local), dist.get_world_size(), rig.j0, rig.j1, n2),
+              file=sys.stderr, flush=True)
 
     def barrier():
         if world > 1:
